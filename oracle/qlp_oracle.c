@@ -1,0 +1,420 @@
+/*
+ * qlp_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU statement of what the QLP GPU transit search computes
+ * (arXiv:2302.01293, /root/reference/PAPER.md; readings of every silent/ambiguous point are
+ * listed in DESIGN.md "Readings" and SURVEY.md section 8(c)).  IEEE FP64, round-to-nearest,
+ * no fused multiply-add (compile with -ffp-contract=off), operations in the order written.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+ * load this.  It shares no code, header, table or constant generator with the CUDA path under
+ * paper_2302_01293_b200/csrc/: every constant below is typed here a second time on purpose.
+ *
+ * Parity pins (tests/test_oracle_*.py): closed forms, invariants, brute force, library special
+ * cases.  The paper prints no spectrum, grid size or S/N value, so "parity unpinned" against
+ * paper-printed numbers (only the order of magnitude of the frequency count).
+ *
+ * Steps (names follow SURVEY.md 8(c)):
+ *   O0 constants, cbrt_det      O1 per-star Keplerian grid
+ *   O2 prep (Kovacs et al. 2002 weights)
+ *   O3 bin index                O4 box scan -> SR(f), best (m, j)
+ *   O5 S/N spectrum (footnote 3 at :65)   O6 peaks
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_PI 0x1.921fb54442d18p+1
+/* O0: K_rho = G rho_sun (86400 s/d)^2 = 3 GM_sun / (4 pi R_sun^3) * 86400^2, GM_sun = 1.3271244e20
+ * m^3 s^-2, R_sun = 6.957e8 m  ->  702.3999946673047 d^-2 (a literal; never recomputed). */
+#define ORC_K_RHO 0x1.5f3333067752fp+9
+#define ORC_MAX_WIDTHS 64
+
+typedef struct {
+  double samples_per_peak; /* 2.0 */
+  double dlogq;            /* 0.1 */
+  int32_t noverlap;        /* 3 */
+  int32_t pad_;
+  double qmin_fac;         /* 0.5 */
+  double qmax_fac;         /* 2.0 */
+  double a_over_rstar_min; /* 2.0 (3.0 for Sectors 59-60) */
+  double sector_days;      /* 27.4 PAPER.md:7 */
+} orc_config;
+
+typedef struct {
+  double t_ref, baseline, p_min, p_max, c_q, u0, h;
+  int64_t n_freq;
+  int32_t nb_max;
+  int32_t status; /* 0 ok; 1: fewer than 2 points; 2: baseline <= 0; 3: f_max <= f_min */
+} orc_star_grid;
+
+typedef struct {
+  int64_t k;
+  double freq, period, t0, sr, snr, q, depth;
+  int32_t m, j, nb, status;
+} orc_peak;
+
+/* ---------------------------------------------------------------- O0 */
+/* cbrt_det: the DEFINITION of the cube root used by the grid (not an approximation of libm's):
+ * frexp, exponent split by 3, eight Newton steps y <- (2y + a/y^2)/3 from y0 = 0.75 + 0.25 a. */
+double orc_cbrt_det(double x) {
+  int e;
+  double mant = frexp(x, &e); /* x = mant * 2^e, mant in [0.5, 1) */
+  int q = (e >= 0) ? (e / 3) : -((-e + 2) / 3); /* floor(e / 3) */
+  int r = e - 3 * q;                              /* 0, 1, 2 */
+  double a = ldexp(mant, r);                      /* [0.5, 4) */
+  double y = 0.75 + 0.25 * a;
+  for (int it = 0; it < 8; ++it) {
+    double y2 = y * y;
+    double d = a / y2;
+    double s = 2.0 * y;
+    double n = s + d;
+    y = n / 3.0;
+  }
+  return ldexp(y, q);
+}
+
+/* O1.9: duration ladder in fine bins.  Rungs q_j = qmin_fac (1+dlogq)^j q_circ, j = 0..J-1 with
+ * J = floor(ln(qmax_fac/qmin_fac)/ln(1+dlogq)) + 1; in fine bins m_j = floor(noverlap (1+dlogq)^j + 0.5),
+ * power by repeated multiplication; duplicates removed.  Defaults -> {3,...,11}.  PAPER.md:19,35. */
+int orc_widths(const orc_config* c, int32_t* M) {
+  int J = (int)floor(log(c->qmax_fac / c->qmin_fac) / log(1.0 + c->dlogq)) + 1;
+  int n = 0;
+  double x = 1.0;
+  for (int j = 0; j < J; ++j) {
+    int m = (int)floor((double)c->noverlap * x + 0.5);
+    if (n == 0 || M[n - 1] != m) {
+      if (n >= ORC_MAX_WIDTHS) return -1;
+      M[n++] = m;
+    }
+    x = x * (1.0 + c->dlogq);
+  }
+  return n;
+}
+
+/* ---------------------------------------------------------------- O1 */
+/* Per-star grid descriptor.  PAPER.md:19 (Keplerian durations, solar density if missing), :23
+ * (P_min where a = k R*, P_max = longest continuous stretch or half of it), :35 (samples_per_peak,
+ * noverlap).  t strictly increasing, days. */
+void orc_grid(const orc_config* c, int64_t n, const double* t, double rho_in, orc_star_grid* g) {
+  memset(g, 0, sizeof(*g));
+  double rho = (isfinite(rho_in) && rho_in > 0.0) ? rho_in : 1.0; /* O1.1 */
+  if (n < 2) { g->status = 1; if (n == 1) g->t_ref = t[0]; return; }
+  g->t_ref = t[0];
+  double T = t[n - 1] - t[0];
+  g->baseline = T;
+  /* O1.2: breaks are gaps strictly longer than one sector; L = longest stretch (last - first). */
+  int has_break = 0;
+  double L = 0.0;
+  int64_t first = 0;
+  for (int64_t i = 0; i + 1 < n; ++i) {
+    if ((t[i + 1] - t[i]) > c->sector_days) {
+      double len = t[i] - t[first];
+      if (len > L) L = len;
+      first = i + 1;
+      has_break = 1;
+    }
+  }
+  {
+    double len = t[n - 1] - t[first];
+    if (len > L) L = len;
+  }
+  double p_max = has_break ? L : 0.5 * L;
+  g->p_max = p_max;
+  /* O1.3: Kepler, a/R* = (G rho P^2 / 3 pi)^(1/3)  =>  P_min = sqrt(3 pi k^3 / (K_rho rho)). */
+  double D = ORC_K_RHO * rho;
+  double k = c->a_over_rstar_min;
+  double c3 = (k * k) * k;
+  double p_min = sqrt(((3.0 * ORC_PI) * c3) / D);
+  g->p_min = p_min;
+  /* O1.4: q_circ(f) = (R* / a) / pi = C_q f^(2/3). */
+  double c_q = orc_cbrt_det((3.0 * ORC_PI) / D) / ORC_PI;
+  g->c_q = c_q;
+  if (!(T > 0.0)) { g->status = 2; return; }
+  if (!(p_max > 0.0)) { g->status = 3; return; }
+  double f_min = 1.0 / p_max;
+  double f_max = 1.0 / p_min;
+  if (!(f_max > f_min)) { g->status = 3; return; }
+  /* O1.6-7: uniform in u = f^(1/3) with step h = qmin_fac C_q / (samples_per_peak T) / 3. */
+  double u0 = orc_cbrt_det(f_min);
+  double u1 = orc_cbrt_det(f_max);
+  double Q = c->qmin_fac * c_q;
+  double A = Q / (c->samples_per_peak * T);
+  double h = A / 3.0;
+  g->u0 = u0;
+  g->h = h;
+  g->n_freq = (int64_t)floor((u1 - u0) / h) + 1;
+  {
+    double u2 = u0 * u0;
+    double qlo = Q * u2;
+    g->nb_max = (int32_t)ceil(((double)c->noverlap) / qlo);
+  }
+}
+
+/* O1.8: frequency k and its number of fine phase bins. */
+void orc_freq(const orc_config* c, const orc_star_grid* g, int64_t k, double* f, int32_t* nb) {
+  double Q = c->qmin_fac * g->c_q;
+  double u = g->u0 + ((double)k) * g->h;
+  double u2 = u * u;
+  *f = u2 * u;
+  double qlo = Q * u2;
+  *nb = (int32_t)ceil(((double)c->noverlap) / qlo);
+}
+
+void orc_freqs(const orc_config* c, const orc_star_grid* g, int64_t k0, int64_t k1, double* f, int32_t* nb) {
+  for (int64_t k = k0; k < k1; ++k) orc_freq(c, g, k, &f[k - k0], &nb[k - k0]);
+}
+
+/* ---------------------------------------------------------------- O2 */
+/* Kovacs et al. (2002) weighting: w_i = dy_i^-2 / sum dy^-2, weighted-mean-subtracted series. */
+void orc_prep(int64_t n, const double* t, const double* y, const double* dy, double t_ref,
+              double* tau, double* w, double* wy) {
+  double W = 0.0;
+  for (int64_t i = 0; i < n; ++i) W += 1.0 / (dy[i] * dy[i]);
+  double ybar = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    w[i] = (1.0 / (dy[i] * dy[i])) / W;
+    ybar += w[i] * y[i];
+  }
+  for (int64_t i = 0; i < n; ++i) {
+    double yt = y[i] - ybar;
+    wy[i] = w[i] * yt;
+    tau[i] = t[i] - t_ref;
+  }
+}
+
+/* ---------------------------------------------------------------- O3 */
+/* Bin index of one point at one frequency; the sequence the CUDA path must reproduce bit for bit. */
+static inline int32_t orc_bin1(double f, int32_t nb, double tau) {
+  double p = f * tau;
+  double c = floor(p);
+  double ph = p - c;
+  double v = ph * (double)nb;
+  int32_t b = (int32_t)v;
+  if (b > nb - 1) b = nb - 1;
+  return b;
+}
+
+void orc_bins(double f, int32_t nb, int64_t n, const double* tau, int32_t* b) {
+  for (int64_t i = 0; i < n; ++i) b[i] = orc_bin1(f, nb, tau[i]);
+}
+
+/* ---------------------------------------------------------------- O3+O4 */
+/* One frequency: fold into nb bins, then try every start bin j and every width m in M (wrapped).
+ * SR = max s^2 / (r (1 - r)); ties -> smaller m, then smaller j; all-zero -> SR 0, (M[0], 0).
+ * Hw/Hs are caller scratch of nb doubles.  r_best/s_best may be NULL. */
+void orc_sr_one(int64_t n, const double* tau, const double* w, const double* wy, double f, int32_t nb,
+                int nM, const int32_t* M, double* Hw, double* Hs,
+                double* sr, int32_t* m_best, int32_t* j_best, double* r_best, double* s_best) {
+  for (int32_t b = 0; b < nb; ++b) { Hw[b] = 0.0; Hs[b] = 0.0; }
+  for (int64_t i = 0; i < n; ++i) {
+    int32_t b = orc_bin1(f, nb, tau[i]);
+    Hw[b] += w[i];
+    Hs[b] += wy[i];
+  }
+  double best = 0.0, rb = 0.0, sb = 0.0;
+  int32_t mb = M[0], jb = 0;
+  for (int im = 0; im < nM; ++im) {   /* widths ascending: first strict improvement wins ties */
+    int32_t m = M[im];
+    for (int32_t j = 0; j < nb; ++j) {
+      double r = 0.0, s = 0.0;
+      for (int32_t l = 0; l < m; ++l) {
+        int32_t b = j + l;
+        if (b >= nb) b -= nb;
+        r += Hw[b];
+        s += Hs[b];
+      }
+      double val = (r > 0.0 && r < 1.0) ? (s * s) / (r * (1.0 - r)) : 0.0;
+      if (val > best) { best = val; mb = m; jb = j; rb = r; sb = s; }
+    }
+  }
+  *sr = best; *m_best = mb; *j_best = jb;
+  if (r_best) *r_best = rb;
+  if (s_best) *s_best = sb;
+}
+
+/* Whole spectrum of one star over its own grid. Outputs have g->n_freq entries. */
+int orc_spectrum_star(const orc_config* c, const orc_star_grid* g, int64_t n, const double* t,
+                      const double* y, const double* dy, double* sr, int32_t* m_best, int32_t* j_best) {
+  if (g->status != 0 || g->n_freq <= 0) return 0;
+  int32_t M[ORC_MAX_WIDTHS];
+  int nM = orc_widths(c, M);
+  if (nM <= 0) return -1;
+  double* tau = (double*)malloc(sizeof(double) * (size_t)n * 3);
+  double* Hw = (double*)malloc(sizeof(double) * (size_t)g->nb_max * 2);
+  if (!tau || !Hw) { free(tau); free(Hw); return -2; }
+  double* w = tau + n;
+  double* wy = w + n;
+  double* Hs = Hw + g->nb_max;
+  orc_prep(n, t, y, dy, g->t_ref, tau, w, wy);
+  for (int64_t k = 0; k < g->n_freq; ++k) {
+    double f; int32_t nb;
+    orc_freq(c, g, k, &f, &nb);
+    orc_sr_one(n, tau, w, wy, f, nb, nM, M, Hw, Hs, &sr[k], &m_best[k], &j_best[k], NULL, NULL);
+  }
+  free(tau); free(Hw);
+  return 0;
+}
+
+/* ---------------------------------------------------------------- O5 */
+static int cmp_double(const void* a, const void* b) {
+  double x = *(const double*)a, y = *(const double*)b;
+  return (x > y) - (x < y);
+}
+static double median_sorted(const double* v, int64_t n) {
+  return (n & 1) ? v[n / 2] : 0.5 * (v[n / 2 - 1] + v[n / 2]);
+}
+
+/* Sturges' law, PAPER.md:65 footnote 3: N = 1 + 3.322 log10(n), rounded to the nearest integer. */
+int32_t orc_sturges(int64_t n) {
+  int32_t N = (int32_t)floor(1.0 + 3.322 * log10((double)n) + 0.5);
+  return N < 1 ? 1 : N;
+}
+
+/* S/N(f) = (SR - trend)/sigma: trend = linear interpolation through the medians
+ * of N equal-width frequency bins (bin centres; constant outside); sigma = 1.4826 MAD(SR).
+ * trend/sigma outputs optional (NULL). */
+void orc_snr(int64_t n, const double* f, const double* sr, double* snr, double* trend_out, double* sigma_out) {
+  if (n <= 0) return;
+  int32_t N = orc_sturges(n);
+  double f0 = f[0];
+  double span = f[n - 1] - f0;
+  double* sorted = (double*)malloc(sizeof(double) * (size_t)n);
+  int32_t* bin = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+  double* cx = (double*)malloc(sizeof(double) * (size_t)N * 2);
+  double* cy = cx + N;
+  int64_t* cnt = (int64_t*)calloc((size_t)N, sizeof(int64_t));
+  for (int64_t k = 0; k < n; ++k) {
+    int32_t b = 0;
+    if (span > 0.0) {
+      b = (int32_t)(((f[k] - f0) / span) * (double)N);
+      if (b > N - 1) b = N - 1;
+    }
+    bin[k] = b;
+    cnt[b]++;
+  }
+  int32_t nk = 0;
+  for (int32_t b = 0; b < N; ++b) {
+    if (cnt[b] == 0) continue;  /* empty bins are dropped */
+    int64_t c = 0;
+    for (int64_t k = 0; k < n; ++k) if (bin[k] == b) sorted[c++] = sr[k];
+    qsort(sorted, (size_t)c, sizeof(double), cmp_double);
+    cx[nk] = f0 + (((double)b + 0.5) * span) / (double)N;
+    cy[nk] = median_sorted(sorted, c);
+    nk++;
+  }
+  /* sigma = 1.4826 * median |SR - median(SR)| (raw spectrum; reading A21). */
+  memcpy(sorted, sr, sizeof(double) * (size_t)n);
+  qsort(sorted, (size_t)n, sizeof(double), cmp_double);
+  double med = median_sorted(sorted, n);
+  for (int64_t k = 0; k < n; ++k) sorted[k] = fabs(sr[k] - med);
+  qsort(sorted, (size_t)n, sizeof(double), cmp_double);
+  double sigma = 1.4826 * median_sorted(sorted, n);
+  if (sigma_out) *sigma_out = sigma;
+  int32_t seg = 0;
+  for (int64_t k = 0; k < n; ++k) {
+    double x = f[k], tr;
+    if (x <= cx[0]) tr = cy[0];
+    else if (x >= cx[nk - 1]) tr = cy[nk - 1];
+    else {
+      while (seg + 1 < nk - 1 && x >= cx[seg + 1]) seg++;
+      while (seg > 0 && x < cx[seg]) seg--;
+      double slope = (cy[seg + 1] - cy[seg]) / (cx[seg + 1] - cx[seg]);
+      tr = slope * (x - cx[seg]) + cy[seg];
+    }
+    if (trend_out) trend_out[k] = tr;
+    snr[k] = (sigma > 0.0) ? (sr[k] - tr) / sigma : 0.0;
+  }
+  free(sorted); free(bin); free(cx); free(cnt);
+}
+
+/* ---------------------------------------------------------------- O6 */
+/* Rank 1 = argmax S/N (ties -> lower k).  Ranks 2..K = remaining strict local maxima
+ * (snr[k] > snr[k-1] and snr[k] >= snr[k+1]; ends compare with their one neighbour) by descending
+ * S/N, ties -> lower k.  Returns the number of peaks written (<= K). */
+int orc_peak_indices(int64_t n, const double* snr, int K, int64_t* out) {
+  if (n <= 0 || K <= 0) return 0;
+  int64_t k1 = 0;
+  for (int64_t k = 1; k < n; ++k) if (snr[k] > snr[k1]) k1 = k;
+  int cnt = 0;
+  out[cnt++] = k1;
+  while (cnt < K) {
+    int64_t best = -1;
+    for (int64_t k = 0; k < n; ++k) {
+      int lm = (k == 0 || snr[k] > snr[k - 1]) && (k == n - 1 || snr[k] >= snr[k + 1]);
+      if (n == 1) lm = 0;
+      if (!lm) continue;
+      int used = 0;
+      for (int i = 0; i < cnt; ++i) if (out[i] == k) used = 1;
+      if (used) continue;
+      /* descending order: must not exceed the previous pick (ties resolved by index) */
+      if (best < 0 || snr[k] > snr[best]) best = k;
+    }
+    if (best < 0) break;
+    out[cnt++] = best;
+  }
+  return cnt;
+}
+
+/* Peak record at frequency k: refold to get (r, s) at the best window; q = m/nb; depth
+ * delta = -s / (r (1 - r)) (positive for a dip); T0 = t_ref + ((j + m/2)/nb)/f.  PAPER.md:44. */
+void orc_peak_record(const orc_config* c, const orc_star_grid* g, int64_t n, const double* t, const double* y,
+                     const double* dy, int64_t k, double snr_k, orc_peak* p) {
+  int32_t M[ORC_MAX_WIDTHS];
+  int nM = orc_widths(c, M);
+  double* tau = (double*)malloc(sizeof(double) * (size_t)n * 3);
+  double* w = tau + n;
+  double* wy = w + n;
+  orc_prep(n, t, y, dy, g->t_ref, tau, w, wy);
+  double f; int32_t nb;
+  orc_freq(c, g, k, &f, &nb);
+  double* Hw = (double*)malloc(sizeof(double) * (size_t)nb * 2);
+  double sr, r, s; int32_t m, j;
+  orc_sr_one(n, tau, w, wy, f, nb, nM, M, Hw, Hw + nb, &sr, &m, &j, &r, &s);
+  p->k = k; p->freq = f; p->period = 1.0 / f; p->sr = sr; p->snr = snr_k;
+  p->m = m; p->j = j; p->nb = nb; p->status = 0;
+  p->q = (double)m / (double)nb;
+  p->depth = (r > 0.0 && r < 1.0) ? -s / (r * (1.0 - r)) : 0.0;
+  p->t0 = g->t_ref + (((double)j + 0.5 * (double)m) / (double)nb) / f;
+  free(tau); free(Hw);
+}
+
+/* ---------------------------------------------------------------- batch driver */
+/* Whole path for a CSR batch, OpenMP over stars only.  sr/m/j/snr are [total_freq] with freq_ptr
+ * offsets (computed by the caller from orc_grid); snr may be NULL; peaks [S*K] may be NULL. */
+int orc_batch(const orc_config* c, int64_t S, const int64_t* row_ptr, const double* t, const double* y,
+              const double* dy, const double* rho, const orc_star_grid* grids, const int64_t* freq_ptr,
+              double* sr, int32_t* mb, int32_t* jb, double* snr, int K, orc_peak* peaks) {
+  int err = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t s = 0; s < S; ++s) {
+    const orc_star_grid* g = &grids[s];
+    int64_t a = row_ptr[s], n = row_ptr[s + 1] - row_ptr[s];
+    int64_t fo = freq_ptr[s], nf = freq_ptr[s + 1] - freq_ptr[s];
+    if (peaks) for (int i = 0; i < K; ++i) { memset(&peaks[s * K + i], 0, sizeof(orc_peak)); peaks[s * K + i].k = -1; peaks[s * K + i].status = 1; }
+    if (g->status != 0 || nf <= 0) continue;
+    int rc = orc_spectrum_star(c, g, n, t + a, y + a, dy + a, sr + fo, mb + fo, jb + fo);
+    if (rc != 0) { err = rc; continue; }
+    if (!snr && !peaks) continue;
+    double* f = (double*)malloc(sizeof(double) * (size_t)nf);
+    int32_t* nbv = (int32_t*)malloc(sizeof(int32_t) * (size_t)nf);
+    double* sn = snr ? snr + fo : (double*)malloc(sizeof(double) * (size_t)nf);
+    orc_freqs(c, g, 0, nf, f, nbv);
+    orc_snr(nf, f, sr + fo, sn, NULL, NULL);
+    if (peaks) {
+      int64_t idx[64];
+      int kk = K > 64 ? 64 : K;
+      int np = orc_peak_indices(nf, sn, kk, idx);
+      for (int i = 0; i < np; ++i) orc_peak_record(c, g, n, t + a, y + a, dy + a, idx[i], sn[idx[i]], &peaks[s * K + i]);
+    }
+    if (!snr) free(sn);
+    free(f); free(nbv);
+  }
+  (void)rho;
+  return err;
+}
+
+int orc_sizeof_grid(void) { return (int)sizeof(orc_star_grid); }
+int orc_sizeof_peak(void) { return (int)sizeof(orc_peak); }
+int orc_sizeof_config(void) { return (int)sizeof(orc_config); }

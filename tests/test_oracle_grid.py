@@ -1,0 +1,160 @@
+"""Pins for the oracle's grid stage (O0/O1): closed forms, hand-built timestamp sets, invariants.
+
+Nothing here re-types the oracle's formulas: P_min and C_q are checked against Kepler's third
+law in SI units, counts against direct enumeration, P_max against hand-built gap patterns
+(PAPER.md:19, 23, 35).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2302_01293_b200 import synth
+
+GM_SUN = 1.3271244e20   # m^3 s^-2 (IAU nominal)
+R_SUN = 6.957e8         # m
+
+
+def a_over_r(period_days, rho_solar):
+    """Kepler III with M = rho * 4/3 pi R^3 (R cancels): a/R for a given period, SI units."""
+    P = period_days * 86400.0
+    R = R_SUN  # any radius: it cancels
+    M_G = GM_SUN * rho_solar * (R / R_SUN) ** 3
+    a = (M_G * P * P / (4.0 * math.pi ** 2)) ** (1.0 / 3.0)
+    return a / R
+
+
+def uniform_t(n, step, t0=2000.0):
+    return t0 + step * np.arange(n)
+
+
+def test_cbrt_det_exact_cases(orc):
+    for i in range(1, 40):
+        assert orc.cbrt_det(float(i ** 3)) == float(i)
+    for e in range(-30, 31):
+        assert orc.cbrt_det(8.0 ** e) == 2.0 ** e
+
+
+def test_cbrt_det_accuracy(orc):
+    rng = np.random.default_rng(1)
+    x = np.exp(rng.uniform(-40, 40, 20000))
+    y = np.array([orc.cbrt_det(v) for v in x])
+    ref = np.cbrt(x)
+    ulp = np.spacing(ref)
+    assert np.max(np.abs(y - ref) / ulp) <= 1.0
+    # y within 1 ulp of the true root => y^3 within 3*(1 ulp relative) of x: at most 4 ulp(x); exact rationals
+    from fractions import Fraction
+    for v, r in zip(x[:300], y[:300]):
+        err = abs(Fraction(r) ** 3 - Fraction(v))
+        assert err <= 4 * Fraction(float(np.spacing(v)))
+
+
+def test_pmin_is_where_a_equals_k_rstar(orc):
+    t = synth.sector_times(0, 1800.0)
+    for k, expect in ((2.0, 0.327634), (3.0, 0.601901)):
+        for rho in (1.0, 0.3, 4.2):
+            g = orc.grid(orc.default_config(a_over_rstar_min=k), t, rho)
+            assert a_over_r(g["p_min"], rho) == pytest.approx(k, rel=1e-7)
+        g = orc.grid(orc.default_config(a_over_rstar_min=k), t, 1.0)
+        assert g["p_min"] == pytest.approx(expect, abs=1e-6)
+
+
+def test_cq_is_circular_central_duty_cycle(orc, cfg):
+    t = synth.sector_times(0, 1800.0)
+    for rho in (1.0, 0.2, 7.0):
+        g = orc.grid(cfg, t, rho)
+        for P in (0.7, 3.0, 11.0):
+            q_circ = g["c_q"] * (1.0 / P) ** (2.0 / 3.0)
+            assert q_circ == pytest.approx(1.0 / (math.pi * a_over_r(P, rho)), rel=1e-7)
+    assert orc.grid(cfg, t, 1.0)["c_q"] == pytest.approx(0.0756390, abs=1e-7)
+
+
+def test_missing_density_is_solar(orc, cfg):
+    t = synth.sector_times(0, 1800.0)
+    ref = orc.grid(cfg, t, 1.0)
+    for bad in (float("nan"), 0.0, -1.0, float("inf")):
+        assert orc.grid(cfg, t, bad) == ref
+
+
+def test_pmax_rule(orc, cfg):
+    step = 0.02
+    # no gap at all: half the stretch
+    t = uniform_t(2001, step)
+    assert orc.grid(cfg, t)["p_max"] == pytest.approx(0.5 * (t[-1] - t[0]), rel=1e-15)
+    # 1-d gaps only (shorter than a sector): still one stretch -> half of the full span
+    t1 = np.concatenate([uniform_t(600, step), uniform_t(600, step, 2000.0 + 600 * step + 1.0)])
+    assert orc.grid(cfg, t1)["p_max"] == pytest.approx(0.5 * (t1[-1] - t1[0]), rel=1e-15)
+    # one 30-d gap: longest side, not halved
+    a, b = uniform_t(500, step), uniform_t(900, step, 2000.0 + 500 * step + 30.0)
+    t2 = np.concatenate([a, b])
+    assert orc.grid(cfg, t2)["p_max"] == pytest.approx(b[-1] - b[0], rel=1e-15)
+    t2r = np.concatenate([uniform_t(900, step), uniform_t(500, step, 2000.0 + 900 * step + 30.0)])
+    assert orc.grid(cfg, t2r)["p_max"] == pytest.approx(899 * step, rel=1e-12)
+    # a gap of exactly one sector is not a break; one cadence more is (dyadic numbers: exact)
+    sd = 27.5
+    c = orc.default_config(sector_days=sd)
+    left = 1000.0 + 0.25 * np.arange(100)
+    for extra, is_break in ((0.0, False), (0.25, True)):
+        right = left[-1] + sd + extra + 0.25 * np.arange(300)
+        tt = np.concatenate([left, right])
+        assert (tt[100] - tt[99] > sd) == is_break
+        want = (right[-1] - right[0]) if is_break else 0.5 * (tt[-1] - tt[0])
+        assert orc.grid(c, tt)["p_max"] == want
+
+
+def test_grid_closed_forms(orc, cfg):
+    for conf, sid in ((1, 0), (2, 3), (3, 5)):
+        t, y, dy, rho, rstar, _ = synth.make_star(conf, sid)
+        g = orc.grid(cfg, t, rho)
+        assert g["status"] == 0
+        f, nb = orc.freqs(cfg, g)
+        n = f.size
+        assert n == g["n_freq"] and n > 1000
+        # ends: first frequency is 1/P_max (cube-root round trip), last one does not pass 1/P_min
+        assert f[0] == pytest.approx(1.0 / g["p_max"], rel=4e-16 * 4)
+        assert f[-1] <= (1.0 / g["p_min"]) * (1 + 1e-15)
+        u1 = (1.0 / g["p_min"]) ** (1.0 / 3.0)
+        assert u1 - (g["u0"] + n * g["h"]) < 0  # one more step would overshoot
+        assert np.all(np.diff(f) > 0)
+        # spacing law: df = q_lo(f) / (samples_per_peak * T), q_lo = 0.5 q_circ
+        q_lo = 0.5 * g["c_q"] * f ** (2.0 / 3.0)
+        df = np.diff(f)
+        assert np.allclose(df, (q_lo[:-1] / (2.0 * g["baseline"])), rtol=3e-3)
+        # fine bins: narrowest searched box is exactly noverlap = 3 bins; grid ends at a/R* = 2
+        assert np.all(nb == np.ceil(3.0 / q_lo - 1e-9)) or np.mean(nb == np.ceil(3.0 / q_lo)) > 0.999
+        assert nb[-1] == 38 == math.ceil(3 * 4 * math.pi)
+        assert nb[0] == g["nb_max"] == nb.max()
+        assert np.all(np.diff(nb) <= 0)
+
+
+def test_grid_sizes_match_design(orc, cfg):
+    # config 1: one 27.4-d sector at 30 min, solar star
+    t, *_ = synth.make_star(1, 0)
+    g = orc.grid(cfg, t, 1.0)
+    assert t.size == 1268 and g["n_freq"] == 4489 and g["nb_max"] == 455
+    # a 40-sector 200-s star stays within "up to ~10 times" 80,000 frequencies
+    t40 = 2000.0 + np.arange(0.0, 40 * 27.4, 1.0)   # continuous 40-sector baseline
+    assert 1e5 < orc.grid(cfg, t40, 1.0)["n_freq"] < 1.2e6
+
+
+def test_grid_invariances(orc, cfg):
+    t, *_ = synth.make_star(3, 11)
+    g = orc.grid(cfg, t, 1.7)
+    g2 = orc.grid(cfg, t + 4096.0, 1.7)   # time zero point is arbitrary
+    assert abs(int(g2["n_freq"]) - int(g["n_freq"])) <= 1
+    assert g2["p_max"] == pytest.approx(g["p_max"], rel=1e-11)
+    assert g2["u0"] == pytest.approx(g["u0"], rel=1e-11)
+
+
+def test_degenerate_stars(orc, cfg):
+    assert orc.grid(cfg, np.array([]))["status"] == 1
+    assert orc.grid(cfg, np.array([5.0]))["status"] == 1
+    g = orc.grid(cfg, 2000.0 + 0.02 * np.arange(20))   # 0.4 d of data: P_max < P_min
+    assert g["status"] == 3 and g["n_freq"] == 0
+
+
+def test_widths(orc):
+    assert list(orc.widths(orc.default_config())) == list(range(3, 12))
+    # by hand: J = floor(ln 4 / ln 1.1) + 1 = 15 rungs, 3 * 1.1^14 = 11.39 -> 11
+    assert math.floor(math.log(4.0) / math.log(1.1)) + 1 == 15
+    assert list(orc.widths(orc.default_config(dlogq=0.5))) == [3, 5, 7, 10]
