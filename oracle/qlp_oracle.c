@@ -185,15 +185,24 @@ void orc_prep(int64_t n, const double* t, const double* y, const double* dy, dou
 }
 
 /* ---------------------------------------------------------------- O3 */
-/* Bin index of one point at one frequency; the sequence the CUDA path must reproduce bit for bit. */
+/* Bin index of one point at one frequency; what the CUDA path must reproduce bit for bit.
+ * Reading A17: p = fl64(f * tau) is the one rounded operation; the bin is then
+ *   b = floor( nb * (p - floor(p)) )   evaluated EXACTLY (no second rounding, hence b <= nb-1
+ * always and no clamp).  p - floor(p) is exact in FP64; its product with the integer nb needs up to
+ * 53 + 15 bits, so it is formed in 128-bit integer arithmetic: ph = M * 2^-sh with M a 53-bit
+ * integer, b = (M * nb) >> sh.  Requires 0 <= p < 2^52 (tau >= 0, f > 0). */
 static inline int32_t orc_bin1(double f, int32_t nb, double tau) {
   double p = f * tau;
   double c = floor(p);
-  double ph = p - c;
-  double v = ph * (double)nb;
-  int32_t b = (int32_t)v;
-  if (b > nb - 1) b = nb - 1;
-  return b;
+  double ph = p - c;                 /* exact, in [0, 1) */
+  if (ph <= 0.0) return 0;
+  int e;
+  double mant = frexp(ph, &e);       /* ph = mant * 2^e, mant in [0.5, 1), e <= 0 */
+  uint64_t M = (uint64_t)ldexp(mant, 53);          /* integer, < 2^53 */
+  int sh = 53 - e;                   /* ph = M * 2^-sh, sh >= 53 */
+  unsigned __int128 prod = (unsigned __int128)M * (unsigned __int128)(uint32_t)nb;
+  if (sh >= 128) return 0;
+  return (int32_t)(uint64_t)(prod >> sh);
 }
 
 void orc_bins(double f, int32_t nb, int64_t n, const double* tau, int32_t* b) {

@@ -15,23 +15,42 @@ from paper_2302_01293_b200 import synth
 
 # ------------------------------------------------------------------ O3: bin index
 def test_bin_index_against_exact_rationals(orc):
+    """O3 (reading A17): b = floor(nb * frac(p)) exactly, p = fl64(f * tau) the only rounding.
+    Checked on every point with Python rationals; and against the exact (unrounded) product f*tau
+    wherever that is not within 1e-9 bin of an edge (the rounding of p cannot matter there)."""
     rng = np.random.default_rng(7)
     tau = np.sort(rng.uniform(0.0, 400.0, 4000))
     checked = 0
-    for f, nb in ((0.0731, 433), (0.91, 97), (3.05, 38), (1.0 / 3.0, 150)):
+    for f, nb in ((0.0731, 433), (0.91, 97), (3.05, 38), (1.0 / 3.0, 150), (16.7, 38), (0.0056, 7814)):
         b = orc.bins(f, nb, tau)
         assert b.min() >= 0 and b.max() <= nb - 1
-        for i in range(0, tau.size, 7):
-            p = Fraction(float(f)) * Fraction(float(tau[i]))       # exact product of the two doubles
-            x = (p - math.floor(p)) * nb
+        for i in range(0, tau.size, 3):
+            p = Fraction(float(f) * float(tau[i]))                  # the rounded FP64 product, exactly
+            assert b[i] == math.floor((p - math.floor(p)) * nb)
+            pe = Fraction(float(f)) * Fraction(float(tau[i]))       # exact product of the two doubles
+            x = (pe - math.floor(pe)) * nb
             if min(x - math.floor(x), math.ceil(x) - x) > Fraction(1, 10 ** 9):   # away from a bin edge
                 assert b[i] == math.floor(x)
                 checked += 1
-    assert checked > 2000
+    assert checked > 6000
+
+
+def test_bin_index_no_double_rounding(orc):
+    """The case that separates the exact floor from floor(fl64(ph*nb)): ph*nb just below an integer."""
+    ph = np.nextafter(1.0, 0.0)                  # 1 - 2^-53
+    for nb in (38, 91, 455, 7814):
+        assert orc.bins(1.0, nb, np.array([ph]))[0] == nb - 1
+    # ph = (n - eps)/nb with eps tiny: fl64(ph*nb) may round up to n, the exact floor is n-1 or n
+    rng = np.random.default_rng(11)
+    for nb in (97, 433):
+        for n in rng.integers(1, nb, 200):
+            ph = np.nextafter(float(n) / nb, 0.0)
+            want = math.floor(Fraction(ph) * nb)
+            assert orc.bins(1.0, nb, np.array([ph]))[0] == want
 
 
 def test_bin_index_edges(orc):
-    # integer phase -> bin 0; phase just below 1 -> last bin (clamped if the product rounds to nb)
+    # integer phase -> bin 0; phase just below 1 -> last bin (exact floor: never reaches nb)
     tau = np.array([0.0, 1.0, 2.0, 4.0, 0.5, 0.25, np.nextafter(1.0, 0.0), np.nextafter(3.0, 0.0)])
     b = orc.bins(1.0, 40, tau)
     assert list(b) == [0, 0, 0, 0, 20, 10, 39, 39]
