@@ -1,0 +1,185 @@
+/*
+ * qlp_bls.h -- C ABI of the B200-native QLP transit-search hot path.
+ *
+ * What it computes: the Box Least Squares spectrum (Kovacs et al. 2002; named as the search
+ * algorithm at) of many ragged TESS light curves over a per-star Keplerian
+ * frequency / duration grid, the paper's S/N spectrum (PAPER.md:37-42,
+ * Eq. 1 and footnote 3 at :65) and the top peaks.  Paper = arXiv:2302.01293,
+ * "QLP Data Release Notes 003: GPU-based Transit Search".  Where the paper is silent the readings
+ * of DESIGN.md ("Readings", A1..A26) apply; the step names S0..S4 / O0..O6 are DESIGN.md's.
+ *
+ * Conventions for every entry point
+ *   - "dev" pointers are CUDA device memory on the context's device, "host" pointers are host
+ *     memory.  All arrays are caller-owned; the library reads inputs, writes outputs and keeps no
+ *     pointer after the call returns.  The context owns only its own workspace.
+ *   - Work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).
+ *     Only qlp_bls_grid() synchronises the stream (to return two totals to the host).
+ *   - Return value: 0 on success, negative qlp_bls_status otherwise.  No exceptions, no aborts,
+ *     nothing written to stdout/stderr.  Data-dependent degeneracy is not an error: a star with
+ *     fewer than two points, zero baseline or P_max <= P_min gets grid.status != 0, n_freq = 0 and
+ *     empty outputs.
+ *   - A context is not thread-safe; use one per host thread / stream.
+ *   - Layout: ragged CSR over stars.  Points: row_ptr[S+1] (int64), star s owns
+ *     [row_ptr[s], row_ptr[s+1]).  Frequencies: freq_ptr[S+1] (int64), ascending frequency within
+ *     a star.  t in days (any zero point), strictly increasing within a star; y any linear flux
+ *     unit; dy > 0.  rho in solar units (non-finite or <= 0 means "solar").
+ */
+#ifndef QLP_BLS_H_
+#define QLP_BLS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qlp_bls_ctx qlp_bls_ctx; /* opaque, owned by the library */
+
+enum qlp_bls_status {
+  QLP_BLS_OK = 0,
+  QLP_BLS_EINVAL = -1,       /* NULL pointer, negative size, bad config field                   */
+  QLP_BLS_ENOMEM = -2,       /* workspace allocation failed                                      */
+  QLP_BLS_ECUDA = -3,        /* a CUDA runtime call or kernel launch failed                      */
+  QLP_BLS_EUNSUPPORTED = -4, /* e.g. a star needs more phase bins than QLP_BLS_MAX_NB            */
+  QLP_BLS_EVALIDATION = -5   /* flags bit0 set and an input failed validation                    */
+};
+
+/* Largest number of fine phase bins per frequency (two FP32 histograms of one frequency must fit
+ * one SM's shared memory; reading A16).  Not reached for rho* <= 30, P <= 180 d. */
+#define QLP_BLS_MAX_NB 24576
+
+/* Search parameters.  POD, caller-owned, copied by qlp_bls_create().  Defaults = the paper's. */
+typedef struct {
+  uint32_t struct_bytes;    /* = sizeof(qlp_bls_config), for versioning                          */
+  int32_t device;           /* CUDA device ordinal                                               */
+  double samples_per_peak;  /* 2.0                                                 */
+  double dlogq;             /* 0.1                                                 */
+  int32_t noverlap;         /* 3                                                 */
+  int32_t top_k;            /* peaks reported per star, 1..8                                     */
+  double qmin_fac;          /* 0.5   PAPER.md:19 ("between 0.5 and 2.0 times" the circular one)  */
+  double qmax_fac;          /* 2.0                                                 */
+  double a_over_rstar_min;  /* 2.0 (3.0 = the Sectors 59-60 variant)                */
+  double sector_days;       /* 27.4                                                  */
+  uint32_t flags;           /* bit0: validate inputs on the device; other bits reserved (0)      */
+  uint32_t reserved_;       /* 0                                                                 */
+} qlp_bls_config;
+
+/* Per-star grid descriptor, written by qlp_bls_grid() (device memory, one per star).
+ * Frequency k of the star is f_k = u^3 with u = u0 + k*h (FP64, in that order), and its number
+ * of fine phase bins is nb_k = ceil(noverlap / (qmin_fac * c_q * u^2)).  DESIGN.md O1. */
+typedef struct {
+  double t_ref;     /* first timestamp: phase zero point (reading A4)                            */
+  double baseline;  /* T = t_last - t_first, days                                                */
+  double p_min;     /* period at which a = a_over_rstar_min * R*   PAPER.md:23                    */
+  double p_max;     /* longest continuous stretch, or half of it                    */
+  double c_q;       /* q_circ(f) = c_q * f^(2/3)                    */
+  double u0;        /* cbrt_det(1 / p_max)                                                       */
+  double h;         /* grid step in u = f^(1/3)                    PAPER.md:35 (samples_per_peak) */
+  int64_t n_freq;   /* number of trial frequencies                                               */
+  int32_t nb_max;   /* phase bins at k = 0 (the largest)                                         */
+  int32_t status;   /* 0 ok; 1 fewer than 2 points; 2 baseline <= 0; 3 f_max <= f_min;
+                       4 nb_max > QLP_BLS_MAX_NB (star skipped, n_freq = 0)                      */
+} qlp_bls_star_grid;
+
+/* One peak of one star, written by qlp_bls_snr() (device memory, [S * top_k], rank-major within
+ * a star).  Unused slots have k = -1, status = 1.  PAPER.md:44 (period, epoch, depth, duration
+ * are what the next pipeline stage takes from the BLS). */
+typedef struct {
+  int64_t k;       /* frequency index within the star's grid                                     */
+  double freq;     /* d^-1                                                                       */
+  double period;   /* d                                                                          */
+  double t0;       /* mid-transit epoch, same zero point as t                                    */
+  float sr;        /* SR at k                                                                    */
+  float snr;       /* S/N at k  (Eq. 1)                                          */
+  float q;         /* m / nb : best duty cycle                                                   */
+  float depth;     /* -s / (r (1 - r)): positive for a dip                                       */
+  int32_t m;       /* best box width in fine bins                                                */
+  int32_t j;       /* best box start bin                                                         */
+  int32_t nb;      /* fine bins at k                                                             */
+  int32_t status;  /* 0 = valid                                                                  */
+} qlp_bls_peak;
+
+/* Fill *cfg with the paper's defaults, device 0, top_k 3. */
+void qlp_bls_default_config(qlp_bls_config* cfg /*host*/);
+
+/* Create a context on cfg->device.  Returns EINVAL for out-of-range fields (noverlap < 1,
+ * widths not inside [1, 31], top_k outside 1..8, non-positive factors), ECUDA if the device
+ * cannot be used. */
+int qlp_bls_create(const qlp_bls_config* cfg /*host*/, qlp_bls_ctx** out /*host*/);
+
+/* S1, per-star Keplerian grid (O1).
+ *   in : row_ptr dev int64[S+1]; t dev double[row_ptr[S]]; rho, rstar dev double[S]
+ *        (rstar may be NULL: it cancels, reading A8).
+ *   out: grid dev [S]; freq_ptr dev int64[S+1] (exclusive scan of n_freq);
+ *        *total_freq = freq_ptr[S] and *total_bins = sum over all frequencies of nb_k (host).
+ * Synchronises the stream. */
+int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                 const double* rho, const double* rstar, qlp_bls_star_grid* grid, int64_t* freq_ptr,
+                 int64_t* total_freq, int64_t* total_bins, void* cuda_stream);
+
+/* S0 + S2 + S3: weights and centred series (Kovacs 2002 weighting), fold-and-bin
+ * at every grid frequency, box scan over every start bin and every width of the duration ladder
+ * (PAPER.md:19, :35).  DESIGN.md O2-O4.
+ *   in : as qlp_bls_grid plus y, dy dev double[row_ptr[S]], and grid / freq_ptr from qlp_bls_grid.
+ *   out: sr dev float[total_freq]   SR(f) = max over boxes of s^2 / (r (1 - r));
+ *        best dev uint32[total_freq] = (m << 24) | j  of the maximising box. */
+int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                     const double* y, const double* dy, const qlp_bls_star_grid* grid,
+                     const int64_t* freq_ptr, float* sr, uint32_t* best, void* cuda_stream);
+
+/* S4: the paper's S/N spectrum (median-binned trend, interpolated and subtracted,
+ * sigma = 1.4826 MAD; bin count by Sturges' law, footnote 3 at :65) and the top_k peaks with
+ * period, epoch, depth, duration.  DESIGN.md O5-O6.
+ *   in : as qlp_bls_spectrum plus its outputs sr, best.
+ *   out: snr dev float[total_freq] or NULL; peaks dev [S * top_k]. */
+int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                const double* y, const double* dy, const qlp_bls_star_grid* grid,
+                const int64_t* freq_ptr, const float* sr, const uint32_t* best, float* snr,
+                qlp_bls_peak* peaks, void* cuda_stream);
+
+/* Whole path with HOST buffers (pageable or pinned): copies the batch to the device, runs
+ * grid -> spectrum -> snr, copies the peak table (and nothing else) back.  This is the call the
+ * end-to-end benchmark times.  peaks host [S * top_k]; grid_out host [S] or NULL. */
+int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                        const double* y, const double* dy, const double* rho, const double* rstar,
+                        qlp_bls_peak* peaks, qlp_bls_star_grid* grid_out, int64_t* total_freq,
+                        void* cuda_stream);
+
+/* Release the context and its workspace.  NULL is allowed. */
+int qlp_bls_destroy(qlp_bls_ctx* ctx);
+
+/* Static string for a status code. */
+const char* qlp_bls_strerror(int code);
+
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+int64_t qlp_bls_launch_count(const qlp_bls_ctx* ctx);
+
+/* The duration ladder in fine bins (O1.9): writes up to cap widths to m (host),
+ * returns their number. */
+int qlp_bls_widths(const qlp_bls_ctx* ctx, int32_t* m /*host*/, int32_t cap);
+
+/* ---- test-only entry points (parity tests call them through the same ABI) ---- */
+
+/* f_k and nb_k for k in [k0, k1) of one star.  grid dev [S]; f dev double[k1-k0]; nb dev int32[k1-k0]. */
+int qlp_bls_debug_freqs(qlp_bls_ctx* ctx, const qlp_bls_star_grid* grid, int64_t star, int64_t k0,
+                        int64_t k1, double* f, int32_t* nb, void* cuda_stream);
+
+/* Bin index (O3) of every point of one star at grid frequency k, computed with the same
+ * device function the fold kernels use.  bin_of_point dev int32[N_star]. */
+int qlp_bls_debug_bins(qlp_bls_ctx* ctx, const int64_t* row_ptr, const double* t,
+                       const qlp_bls_star_grid* grid, int64_t star, int64_t k, int32_t* bin_of_point,
+                       void* cuda_stream);
+
+/* S0 outputs of one star: tau dev double[N], w dev float[N], wy dev float[N]. */
+int qlp_bls_debug_prep(qlp_bls_ctx* ctx, const int64_t* row_ptr, const double* t, const double* y,
+                       const double* dy, const qlp_bls_star_grid* grid, int64_t star, double* tau,
+                       float* w, float* wy, void* cuda_stream);
+
+/* Force one fold kernel for all frequencies: 0 = automatic (default), 1 = column kernel only
+ * where it fits else wide, 2 = wide kernel everywhere.  Used by parity tests to cover both. */
+int qlp_bls_debug_set_path(qlp_bls_ctx* ctx, int32_t path);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QLP_BLS_H_ */

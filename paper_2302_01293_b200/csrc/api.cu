@@ -1,0 +1,404 @@
+// api.cu -- the C ABI of include/qlp_bls.h: context, workspace and kernel launches.
+// Every step of the path runs in the kernels of grid.cuh / prep.cuh / foldscan.cuh / snr_kernel.cuh;
+// the host code below only sizes buffers and enqueues work.
+#include <math.h>
+#include <new>
+#include <string.h>
+
+#include "common.cuh"
+#include "foldscan.cuh"
+#include "grid.cuh"
+#include "prep.cuh"
+#include "snr_kernel.cuh"
+
+using namespace qlp;
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t cap = 0;
+  int ensure(size_t bytes) {
+    if (bytes <= cap) return 0;
+    if (p) cudaFree(p);
+    p = nullptr; cap = 0;
+    size_t want = bytes + bytes / 8 + 256;
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e != cudaSuccess) { cudaGetLastError(); e = cudaMalloc(&p, bytes); want = bytes; }
+    if (e != cudaSuccess) { cudaGetLastError(); p = nullptr; return QLP_BLS_ENOMEM; }
+    cap = want;
+    return 0;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+struct qlp_bls_ctx {
+  qlp_bls_config cfg;
+  Params prm;
+  int device = 0;
+  int n_sm = 148;
+  int32_t widths[32];
+  int n_widths = 0;
+  int32_t force_path = 0;
+  int64_t launches = 0;
+  // workspace
+  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev;
+  // host-API staging
+  DevBuf h_row, h_t, h_y, h_dy, h_rho, h_grid, h_fptr, h_sr, h_best, h_peaks;
+  int64_t* totals_host = nullptr;  // pinned, 4 x int64
+  // cache of the last grid call: lets spectrum/snr size the point workspace without a sync
+  const int64_t* last_row_ptr = nullptr;
+  int64_t last_n_stars = -1, last_n_points = -1;
+};
+
+#define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { cudaGetLastError(); return QLP_BLS_ECUDA; } } while (0)
+#define QLP_TRY(x) do { int r_ = (x); if (r_ != 0) return r_; } while (0)
+
+static int launch_ok(qlp_bls_ctx* ctx) {
+  ctx->launches++;
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 0 : QLP_BLS_ECUDA;
+}
+
+extern "C" void qlp_bls_default_config(qlp_bls_config* cfg) {
+  if (!cfg) return;
+  memset(cfg, 0, sizeof(*cfg));
+  cfg->struct_bytes = (uint32_t)sizeof(qlp_bls_config);
+  cfg->device = 0;
+  cfg->samples_per_peak = 2.0;
+  cfg->dlogq = 0.1;
+  cfg->noverlap = 3;
+  cfg->top_k = 3;
+  cfg->qmin_fac = 0.5;
+  cfg->qmax_fac = 2.0;
+  cfg->a_over_rstar_min = 2.0;
+  cfg->sector_days = 27.4;
+  cfg->flags = 0;
+}
+
+// O1.9: duration ladder in fine bins.
+static int build_widths(const qlp_bls_config& c, int32_t* M, int cap) {
+  int J = (int)floor(log(c.qmax_fac / c.qmin_fac) / log(1.0 + c.dlogq)) + 1;
+  int n = 0;
+  double x = 1.0;
+  for (int j = 0; j < J; ++j) {
+    int m = (int)floor((double)c.noverlap * x + 0.5);
+    if (n == 0 || M[n - 1] != m) {
+      if (n >= cap) return -1;
+      M[n++] = m;
+    }
+    x = x * (1.0 + c.dlogq);
+  }
+  return n;
+}
+
+extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
+  if (!cfg || !out) return QLP_BLS_EINVAL;
+  *out = nullptr;
+  if (cfg->struct_bytes != sizeof(qlp_bls_config)) return QLP_BLS_EINVAL;
+  if (!(cfg->samples_per_peak > 0.0) || !(cfg->dlogq > 0.0) || cfg->noverlap < 1 || cfg->noverlap > kMaxWidth ||
+      !(cfg->qmin_fac > 0.0) || !(cfg->qmax_fac >= cfg->qmin_fac) || !(cfg->a_over_rstar_min > 0.0) ||
+      !(cfg->sector_days > 0.0) || cfg->top_k < 1 || cfg->top_k > kMaxTopK)
+    return QLP_BLS_EINVAL;
+  qlp_bls_ctx* ctx = new (std::nothrow) qlp_bls_ctx();
+  if (!ctx) return QLP_BLS_ENOMEM;
+  ctx->cfg = *cfg;
+  ctx->n_widths = build_widths(*cfg, ctx->widths, 32);
+  if (ctx->n_widths <= 0) { delete ctx; return QLP_BLS_EINVAL; }
+  Params& p = ctx->prm;
+  p.samples_per_peak = cfg->samples_per_peak; p.dlogq = cfg->dlogq; p.qmin_fac = cfg->qmin_fac;
+  p.qmax_fac = cfg->qmax_fac; p.a_over_rstar_min = cfg->a_over_rstar_min; p.sector_days = cfg->sector_days;
+  p.noverlap = cfg->noverlap; p.top_k = cfg->top_k;
+  p.wmask = 0; p.max_width = 0; p.min_width = ctx->widths[0];
+  for (int i = 0; i < ctx->n_widths; ++i) {
+    int m = ctx->widths[i];
+    if (m < 1 || m > kMaxWidth) { delete ctx; return QLP_BLS_EINVAL; }
+    p.wmask |= 1u << m;
+    if (m > p.max_width) p.max_width = m;
+    if (m < p.min_width) p.min_width = m;
+  }
+  // every box must be narrower than the coarsest histogram: nb >= noverlap pi a_min / qmin_fac
+  if (!((double)cfg->noverlap * QLP_PI * cfg->a_over_rstar_min / cfg->qmin_fac > (double)p.max_width + 1.0)) {
+    delete ctx; return QLP_BLS_EINVAL;
+  }
+  ctx->device = cfg->device;
+  if (cudaSetDevice(ctx->device) != cudaSuccess) { cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA; }
+  int n_sm = 0;
+  if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, ctx->device) != cudaSuccess || n_sm <= 0) {
+    cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
+  }
+  ctx->n_sm = n_sm;
+  const int max_smem = 227 * 1024;
+  if (cudaFuncSetAttribute(foldscan_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(foldscan_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
+    cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
+  }
+  if (cudaMallocHost((void**)&ctx->totals_host, 4 * sizeof(int64_t)) != cudaSuccess) {
+    cudaGetLastError(); delete ctx; return QLP_BLS_ENOMEM;
+  }
+  if (ctx->totals_dev.ensure(4 * sizeof(int64_t)) != 0) { cudaFreeHost(ctx->totals_host); delete ctx; return QLP_BLS_ENOMEM; }
+  *out = ctx;
+  return QLP_BLS_OK;
+}
+
+extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
+  if (!ctx) return QLP_BLS_OK;
+  cudaSetDevice(ctx->device);
+  DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
+                    &ctx->totals_dev, &ctx->h_row, &ctx->h_t, &ctx->h_y, &ctx->h_dy, &ctx->h_rho, &ctx->h_grid,
+                    &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks};
+  for (DevBuf* b : bufs) b->release();
+  if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
+  delete ctx;
+  return QLP_BLS_OK;
+}
+
+extern "C" const char* qlp_bls_strerror(int code) {
+  switch (code) {
+    case QLP_BLS_OK: return "ok";
+    case QLP_BLS_EINVAL: return "invalid argument";
+    case QLP_BLS_ENOMEM: return "out of memory";
+    case QLP_BLS_ECUDA: return "CUDA error";
+    case QLP_BLS_EUNSUPPORTED: return "unsupported";
+    case QLP_BLS_EVALIDATION: return "input validation failed";
+    default: return "unknown status";
+  }
+}
+
+extern "C" int64_t qlp_bls_launch_count(const qlp_bls_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int qlp_bls_widths(const qlp_bls_ctx* ctx, int32_t* m, int32_t cap) {
+  if (!ctx || !m) return QLP_BLS_EINVAL;
+  int n = ctx->n_widths < cap ? ctx->n_widths : cap;
+  for (int i = 0; i < n; ++i) m[i] = ctx->widths[i];
+  return ctx->n_widths;
+}
+
+extern "C" int qlp_bls_debug_set_path(qlp_bls_ctx* ctx, int32_t path) {
+  if (!ctx || path < 0 || path > 3) return QLP_BLS_EINVAL;
+  ctx->force_path = path;
+  return QLP_BLS_OK;
+}
+
+// ---- S1 -----------------------------------------------------------------------------------------
+extern "C" int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                            const double* rho, const double* rstar, qlp_bls_star_grid* grid, int64_t* freq_ptr,
+                            int64_t* total_freq, int64_t* total_bins, void* cuda_stream) {
+  (void)rstar;  // R* cancels out of a/R* = (G rho P^2 / 3 pi)^(1/3): DESIGN.md reading A8
+  if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr || !total_freq || !total_bins) return QLP_BLS_EINVAL;
+  if (n_stars > 0 && (!t || !rho || !grid)) return QLP_BLS_EINVAL;
+  if (n_stars > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  QLP_TRY(ctx->star_bins.ensure((size_t)(n_stars + 1) * 8));
+  if (n_stars > 0) {
+    grid_kernel<<<(unsigned)n_stars, 256, 0, st>>>(ctx->prm, n_stars, row_ptr, t, rho, grid,
+                                                  (unsigned long long*)ctx->star_bins.p);
+    QLP_TRY(launch_ok(ctx));
+  }
+  int64_t* totals = (int64_t*)ctx->totals_dev.p;
+  freq_scan_kernel<<<1, 1024, 0, st>>>(n_stars, grid, (const unsigned long long*)ctx->star_bins.p, freq_ptr, totals);
+  QLP_TRY(launch_ok(ctx));
+  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host, totals, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 2, row_ptr + n_stars, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  *total_freq = ctx->totals_host[0];
+  *total_bins = ctx->totals_host[1];
+  ctx->last_row_ptr = row_ptr; ctx->last_n_stars = n_stars; ctx->last_n_points = ctx->totals_host[2];
+  return QLP_BLS_OK;
+}
+
+// number of points of the batch: cached by qlp_bls_grid, else one small synchronising read-back
+static int batch_points(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, cudaStream_t st, int64_t* n_points) {
+  if (ctx->last_row_ptr == row_ptr && ctx->last_n_stars == n_stars && ctx->last_n_points >= 0) {
+    *n_points = ctx->last_n_points;
+    return 0;
+  }
+  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 2, row_ptr + n_stars, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  *n_points = ctx->totals_host[2];
+  ctx->last_row_ptr = row_ptr; ctx->last_n_stars = n_stars; ctx->last_n_points = *n_points;
+  return 0;
+}
+
+// S0 into the context workspace
+static int run_prep(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
+                    const double* dy, const qlp_bls_star_grid* grid, cudaStream_t st) {
+  int64_t n_points = 0;
+  QLP_TRY(batch_points(ctx, n_stars, row_ptr, st, &n_points));
+  if (n_points < 0) return QLP_BLS_EINVAL;
+  QLP_TRY(ctx->pts.ensure((size_t)(n_points + 1) * sizeof(Point)));
+  QLP_TRY(ctx->prep.ensure((size_t)(n_stars + 1) * sizeof(StarPrep)));
+  prep_kernel<<<(unsigned)n_stars, 256, 0, st>>>(ctx->prm, n_stars, row_ptr, t, y, dy, grid, (Point*)ctx->pts.p,
+                                                (StarPrep*)ctx->prep.p);
+  return launch_ok(ctx);
+}
+
+// ---- S0 + S2 + S3 ---------------------------------------------------------------------------------
+extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                const double* y, const double* dy, const qlp_bls_star_grid* grid,
+                                const int64_t* freq_ptr, float* sr, uint32_t* best, void* cuda_stream) {
+  if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr) return QLP_BLS_EINVAL;
+  if (n_stars == 0) return QLP_BLS_OK;
+  if (!t || !y || !dy || !grid || !sr || !best) return QLP_BLS_EINVAL;
+  if (n_stars > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  QLP_TRY(run_prep(ctx, n_stars, row_ptr, t, y, dy, grid, st));
+  QLP_TRY(ctx->kb.ensure((size_t)n_stars * kNumClasses * 8));
+  QLP_TRY(ctx->cnt.ensure((size_t)n_stars * kNumClasses * 8));
+  QLP_TRY(ctx->off.ensure((size_t)(n_stars + 1) * kNumClasses * 8));
+  QLP_TRY(ctx->counters.ensure(kNumClasses * 8));
+  int64_t* kb = (int64_t*)ctx->kb.p;
+  int64_t* cnt = (int64_t*)ctx->cnt.p;
+  int64_t* off = (int64_t*)ctx->off.p;
+  unsigned long long* counters = (unsigned long long*)ctx->counters.p;
+  CUDA_TRY(cudaMemsetAsync(counters, 0, kNumClasses * 8, st));
+  tile_bounds_kernel<<<(unsigned)((n_stars + 127) / 128), 128, 0, st>>>(ctx->prm, n_stars, grid, ctx->force_path, kb, cnt);
+  QLP_TRY(launch_ok(ctx));
+  tile_scan_kernel<<<kNumClasses, 1024, 0, st>>>(n_stars, cnt, off);
+  QLP_TRY(launch_ok(ctx));
+  for (int c = 0; c < kNumClasses; ++c) {
+    const size_t smem = (size_t)class_cols(c) * class_nbcap(c) * 8;
+    const int per_sm = (c == 0) ? 4 : (c == 1 ? 2 : 1);
+    const unsigned nblk = (unsigned)(ctx->n_sm * per_sm);
+    const int64_t* off_c = off + (int64_t)c * (n_stars + 1);
+    if (ctx->prm.max_width <= 11)
+      foldscan_kernel<11><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,
+                                                      (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,
+                                                      counters + c, sr, best);
+    else
+      foldscan_kernel<16><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,
+                                                      (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,
+                                                      counters + c, sr, best);
+    QLP_TRY(launch_ok(ctx));
+  }
+  return QLP_BLS_OK;
+}
+
+// ---- S4 -------------------------------------------------------------------------------------------
+extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
+                           const double* dy, const qlp_bls_star_grid* grid, const int64_t* freq_ptr, const float* sr,
+                           const uint32_t* best, float* snr, qlp_bls_peak* peaks, void* cuda_stream) {
+  if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr) return QLP_BLS_EINVAL;
+  if (n_stars == 0) return QLP_BLS_OK;
+  if (!t || !y || !dy || !grid || !sr || !best || !peaks) return QLP_BLS_EINVAL;
+  if (n_stars > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  QLP_TRY(run_prep(ctx, n_stars, row_ptr, t, y, dy, grid, st));  // one cheap pass; never trusts stale state
+  snr_kernel<<<(unsigned)n_stars, kSnrThreads, kMaxSel * 256 * 4, st>>>(
+      ctx->prm, n_stars, row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, grid, freq_ptr, sr, best,
+      snr, peaks);
+  return launch_ok(ctx);
+}
+
+// ---- whole path from host buffers -------------------------------------------------------------------
+// Stars are processed in chunks bounded by a point budget so that the device copies stay small next
+// to 180 GB of HBM: per chunk H2D (row_ptr rebased, t, y, dy, rho) -> grid -> spectrum -> snr -> D2H
+// of the peak table only.
+extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                   const double* y, const double* dy, const double* rho, const double* rstar,
+                                   qlp_bls_peak* peaks, qlp_bls_star_grid* grid_out, int64_t* total_freq,
+                                   void* cuda_stream) {
+  (void)rstar;
+  if (!ctx || n_stars < 0 || !row_ptr || !peaks) return QLP_BLS_EINVAL;
+  if (n_stars > 0 && (!t || !y || !dy || !rho)) return QLP_BLS_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  const int K = ctx->prm.top_k;
+  const int64_t kPointBudget = 256ll << 20;  // points per chunk (4 GiB of point records)
+  const int64_t kStarBudget = 1 << 20;
+  int64_t tf_sum = 0;
+  int64_t s0 = 0;
+  int64_t* row_tmp = nullptr;
+  while (s0 < n_stars) {
+    int64_t s1 = s0 + 1;
+    while (s1 < n_stars && (row_ptr[s1 + 1] - row_ptr[s0]) <= kPointBudget && (s1 - s0) < kStarBudget) ++s1;
+    const int64_t S = s1 - s0, p0 = row_ptr[s0], np = row_ptr[s1] - p0;
+    if (np < 0) return QLP_BLS_EINVAL;
+    QLP_TRY(ctx->h_row.ensure((size_t)(S + 1) * 8));
+    QLP_TRY(ctx->h_t.ensure((size_t)(np + 1) * 8));
+    QLP_TRY(ctx->h_y.ensure((size_t)(np + 1) * 8));
+    QLP_TRY(ctx->h_dy.ensure((size_t)(np + 1) * 8));
+    QLP_TRY(ctx->h_rho.ensure((size_t)S * 8));
+    QLP_TRY(ctx->h_grid.ensure((size_t)S * sizeof(qlp_bls_star_grid)));
+    QLP_TRY(ctx->h_fptr.ensure((size_t)(S + 1) * 8));
+    QLP_TRY(ctx->h_peaks.ensure((size_t)S * K * sizeof(qlp_bls_peak)));
+    const int64_t* row_src = row_ptr + s0;
+    if (p0 != 0) {  // rebase the chunk's row_ptr to zero
+      row_tmp = (int64_t*)realloc(row_tmp, (size_t)(S + 1) * 8);
+      if (!row_tmp) return QLP_BLS_ENOMEM;
+      for (int64_t i = 0; i <= S; ++i) row_tmp[i] = row_ptr[s0 + i] - p0;
+      row_src = row_tmp;
+    }
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_row.p, row_src, (size_t)(S + 1) * 8, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_t.p, t + p0, (size_t)np * 8, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_y.p, y + p0, (size_t)np * 8, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_dy.p, dy + p0, (size_t)np * 8, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_rho.p, rho + s0, (size_t)S * 8, cudaMemcpyHostToDevice, st));
+    if (row_src == row_tmp) CUDA_TRY(cudaStreamSynchronize(st));  // row_tmp is reused by the next chunk
+    int64_t tf = 0, tb = 0;
+    ctx->last_row_ptr = nullptr;  // staging pointers are reused across chunks: never trust the cache
+    int rc = qlp_bls_grid(ctx, S, (const int64_t*)ctx->h_row.p, (const double*)ctx->h_t.p, (const double*)ctx->h_rho.p,
+                          nullptr, (qlp_bls_star_grid*)ctx->h_grid.p, (int64_t*)ctx->h_fptr.p, &tf, &tb, st);
+    if (rc != 0) { free(row_tmp); return rc; }
+    tf_sum += tf;
+    if ((rc = ctx->h_sr.ensure((size_t)(tf + 1) * 4)) != 0 || (rc = ctx->h_best.ensure((size_t)(tf + 1) * 4)) != 0) {
+      free(row_tmp); return rc;
+    }
+    rc = qlp_bls_spectrum(ctx, S, (const int64_t*)ctx->h_row.p, (const double*)ctx->h_t.p, (const double*)ctx->h_y.p,
+                          (const double*)ctx->h_dy.p, (const qlp_bls_star_grid*)ctx->h_grid.p,
+                          (const int64_t*)ctx->h_fptr.p, (float*)ctx->h_sr.p, (uint32_t*)ctx->h_best.p, st);
+    if (rc == 0)
+      rc = qlp_bls_snr(ctx, S, (const int64_t*)ctx->h_row.p, (const double*)ctx->h_t.p, (const double*)ctx->h_y.p,
+                       (const double*)ctx->h_dy.p, (const qlp_bls_star_grid*)ctx->h_grid.p,
+                       (const int64_t*)ctx->h_fptr.p, (const float*)ctx->h_sr.p, (const uint32_t*)ctx->h_best.p,
+                       nullptr, (qlp_bls_peak*)ctx->h_peaks.p, st);
+    if (rc != 0) { free(row_tmp); return rc; }
+    cudaError_t e = cudaMemcpyAsync(peaks + s0 * K, ctx->h_peaks.p, (size_t)S * K * sizeof(qlp_bls_peak),
+                                    cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && grid_out)
+      e = cudaMemcpyAsync(grid_out + s0, ctx->h_grid.p, (size_t)S * sizeof(qlp_bls_star_grid), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { cudaGetLastError(); free(row_tmp); return QLP_BLS_ECUDA; }
+    s0 = s1;
+  }
+  free(row_tmp);
+  if (total_freq) *total_freq = tf_sum;
+  return QLP_BLS_OK;
+}
+
+// ---- test-only entry points ---------------------------------------------------------------------------
+extern "C" int qlp_bls_debug_freqs(qlp_bls_ctx* ctx, const qlp_bls_star_grid* grid, int64_t star, int64_t k0,
+                                   int64_t k1, double* f, int32_t* nb, void* cuda_stream) {
+  if (!ctx || !grid || star < 0 || k0 < 0 || k1 < k0) return QLP_BLS_EINVAL;
+  if (k1 == k0) return QLP_BLS_OK;
+  if (!f || !nb) return QLP_BLS_EINVAL;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  int64_t nblk = (k1 - k0 + 255) / 256;
+  if (nblk > 4096) nblk = 4096;
+  debug_freqs_kernel<<<(unsigned)nblk, 256, 0, (cudaStream_t)cuda_stream>>>(ctx->prm, grid, star, k0, k1, f, nb);
+  return launch_ok(ctx);
+}
+
+extern "C" int qlp_bls_debug_bins(qlp_bls_ctx* ctx, const int64_t* row_ptr, const double* t,
+                                  const qlp_bls_star_grid* grid, int64_t star, int64_t k, int32_t* bin_of_point,
+                                  void* cuda_stream) {
+  if (!ctx || !row_ptr || !t || !grid || !bin_of_point || star < 0 || k < 0) return QLP_BLS_EINVAL;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  debug_bins_kernel<<<256, 256, 0, (cudaStream_t)cuda_stream>>>(ctx->prm, row_ptr, t, grid, star, k, bin_of_point);
+  return launch_ok(ctx);
+}
+
+extern "C" int qlp_bls_debug_prep(qlp_bls_ctx* ctx, const int64_t* row_ptr, const double* t, const double* y,
+                                  const double* dy, const qlp_bls_star_grid* grid, int64_t star, double* tau, float* w,
+                                  float* wy, void* cuda_stream) {
+  if (!ctx || !row_ptr || !t || !y || !dy || !grid || !tau || !w || !wy || star < 0) return QLP_BLS_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  // the prep kernel runs over the whole batch; the caller passes the batch size through the grid call
+  if (ctx->last_row_ptr != row_ptr || ctx->last_n_stars <= star) return QLP_BLS_EINVAL;
+  QLP_TRY(run_prep(ctx, ctx->last_n_stars, row_ptr, t, y, dy, grid, st));
+  debug_prep_kernel<<<64, 256, 0, st>>>(row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, star, tau, w, wy);
+  return launch_ok(ctx);
+}

@@ -1,0 +1,120 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a only).
+//
+// Nothing here is shared with oracle/: constants and the deterministic cube root are typed a second
+// time on purpose.  Step names (S0..S4, O0..O6) are DESIGN.md's.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/qlp_bls.h"
+
+namespace qlp {
+
+// ---- O0 constants (O0; PAPER.md:19 "stellar density", :7 sector length) -------------
+// pi and K_rho = G rho_sun (86400 s/d)^2 = 3 GM_sun/(4 pi R_sun^3) 86400^2 with the IAU nominal
+// GM_sun = 1.3271244e20 m^3 s^-2, R_sun = 6.957e8 m  ->  702.3999946673047 d^-2.
+#define QLP_PI 3.141592653589793115997963468544185161590576171875
+#define QLP_K_RHO 702.399994667304699760279618203639984130859375
+#define QLP_TWO52 4503599627370496.0
+
+constexpr int kMaxWidth = 16;     // largest supported box width in fine bins (ladder default: 11)
+constexpr int kThreads = 256;     // threads per CTA of the fold/scan kernel
+constexpr int kWarps = kThreads / 32;
+constexpr int kNumClasses = 9;    // tile classes, see foldscan.cu
+constexpr int kMaxTopK = 8;
+constexpr uint32_t kScaleW = 4290772992u;  // 2^32 - 2^22: fixed-point unit of the weights
+
+// One light-curve point as the fold kernel reads it: 16 bytes, one LDG.128 / LDS.128.
+struct __align__(16) Point {
+  double tau;   // t - t_ref (O2)
+  uint32_t W;   // round(w * kScaleW), w = dy^-2 / sum dy^-2
+  int32_t S;    // round(w * (y - ybar) * scale_s)
+};
+
+// Per-star results of S0 that later steps need.
+struct StarPrep {
+  double ybar;      // weighted mean (O2)
+  double wsum;      // sum dy^-2
+  double scale_s;   // fixed-point units per unit of w*ytilde (0 if the series is constant)
+  float inv_w;      // 1 / kScaleW
+  float inv_s;      // 1 / scale_s (0 if scale_s == 0)
+  int32_t status;   // 0 ok, 5: too many points for the fixed-point weights
+  int32_t pad_;
+};
+
+// Resolved search parameters (device copy of qlp_bls_config plus derived values).
+struct Params {
+  double samples_per_peak, dlogq, qmin_fac, qmax_fac, a_over_rstar_min, sector_days;
+  int32_t noverlap, top_k;
+  uint32_t wmask;     // bit m set <=> width m is on the ladder (O1.9)
+  int32_t max_width;  // largest width
+  int32_t min_width;  // smallest width (the all-zero answer, O4)
+};
+
+// One unit of work of the fold/scan kernel: `ncols` consecutive frequencies of one star.
+struct Tile {
+  int32_t star;
+  int32_t ncols;   // <= columns per CTA of the class
+  int64_t k0;      // first frequency index within the star
+};
+
+// ---- exact FP64 helpers: never contracted into FMAs (O1/O3: "no fused multiply-add") ---
+__device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double dadd(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double dsub(double a, double b) { return __dadd_rn(a, -b); }
+__device__ __forceinline__ double ddiv(double a, double b) { return __ddiv_rn(a, b); }
+
+// cbrt_det (O0): frexp, exponent split by 3, eight Newton steps from y0 = 0.75 + 0.25 a.
+__device__ inline double cbrt_det(double x) {
+  int e;
+  double mant = frexp(x, &e);
+  int q = (e >= 0) ? (e / 3) : -((-e + 2) / 3);
+  int r = e - 3 * q;
+  double a = ldexp(mant, r);
+  double y = dadd(0.75, dmul(0.25, a));
+#pragma unroll 1
+  for (int it = 0; it < 8; ++it) {
+    double y2 = dmul(y, y);
+    double d = ddiv(a, y2);
+    double s = dmul(2.0, y);
+    double n = dadd(s, d);
+    y = ddiv(n, 3.0);
+  }
+  return ldexp(y, q);
+}
+
+// O1.8: frequency k of a star and its number of fine bins.  Q = qmin_fac * c_q.
+__device__ __forceinline__ void freq_of_k(double u0, double h, double Q, double noverlap, int64_t k,
+                                          double& f, int32_t& nb) {
+  double u = dadd(u0, dmul((double)k, h));
+  double u2 = dmul(u, u);
+  f = dmul(u2, u);
+  double qlo = dmul(Q, u2);
+  nb = (int32_t)ceil(ddiv(noverlap, qlo));
+}
+
+// O3: bin of one point.  p = fl64(f * tau) is the only rounded operation; the bin is
+// floor(nb * frac(p)) exactly.  Four FP64 instructions:
+//   c' = RD(p + 2^52)           = 2^52 + floor(p)                  (0 <= p < 2^51)
+//   A  = fma(-nb, c', (nb+1) 2^52) = 2^52 - nb floor(p)             (exactly representable)
+//   v  = RD(fma(p, nb, A))      = 2^52 + floor(nb (p - floor p))   (one rounding, downwards)
+// and the low word of v is the bin.  dnb = (double)nb, K = (nb + 1) * 2^52.
+__device__ __forceinline__ int32_t bin_of(double f, double tau, double dnb, double K) {
+  double p = __dmul_rn(f, tau);
+  double c = __dadd_rd(p, QLP_TWO52);
+  double A = __fma_rn(-dnb, c, K);
+  double v = __fma_rd(p, dnb, A);
+  return __double2loint(v);
+}
+
+// Tile classes of the fold/scan kernel: columns per CTA and the largest nb the class holds.
+__host__ __device__ __forceinline__ int class_cols(int c) {
+  return c <= 2 ? 64 : (32 >> (c - 3));
+}
+__host__ __device__ __forceinline__ int class_nbcap(int c) {
+  // shared memory = cols * nbcap * 8 bytes
+  const int caps[kNumClasses] = {110, 220, 440, 880, 1760, 3520, 7040, 14080, 24576};
+  return caps[c];
+}
+
+}  // namespace qlp

@@ -1,0 +1,273 @@
+// foldscan.cuh -- S2 fold-and-bin fused with S3 box-scan (O3, O4; the BLS of Kovacs et
+// al. 2002 that PAPER.md:13 and :37 name, on the Keplerian duration ladder of PAPER.md:19, :35).
+//
+// Work unit ("tile"): one star x `cols` consecutive grid frequencies.  Each frequency owns one
+// COLUMN of two integer histograms in shared memory (sum of W and sum of S per phase bin); a lane of
+// a warp owns one column, so the 32 lanes of a warp fold the SAME point at 32 different
+// frequencies: the point is one broadcast 16-byte load, the 32 accumulations go to 32 different
+// banks, and the two accumulations are native ATOMS.ADD (no return value -> no dependent chain).
+// The warps of the CTA split the point stream; atomics make their concurrent updates safe.
+// After the fold the histograms never leave the SM: the box scan runs on them in place and only
+// SR(f) and the best (m, j) go to HBM (8 bytes per frequency).
+//
+// nb (phase bins) falls from nb_max to ~38 along a star's grid, so tiles come in classes that trade
+// columns for bins within the same shared-memory budget (class_cols / class_nbcap in common.cuh).
+// In the narrow classes (fewer than 32 columns) the spare lanes of a warp take consecutive points.
+// Each class is one persistent launch that pulls tile numbers from an atomic counter; a tile number
+// is mapped to (star, k0) by a binary search in the per-class prefix sums built by tile_bounds_kernel
+// and tile_scan_kernel, so no tile list is materialised.
+#pragma once
+#include "common.cuh"
+
+namespace qlp {
+
+// ---- tile bookkeeping -------------------------------------------------------------------------
+// kb[s][c] = first k of star s whose nb_k <= class_nbcap(c) (n_freq if none); class c then covers
+// k in [kb[s][c], kb[s][c-1]) for c >= 1 and [kb[s][0], n_freq) for c = 0.  nb_k is non-increasing
+// in k because every operation of O1.8 is monotone.
+__global__ void tile_bounds_kernel(Params prm, int64_t n_stars, const qlp_bls_star_grid* __restrict__ grid,
+                                   int32_t force_path, int64_t* __restrict__ kb, int64_t* __restrict__ cnt) {
+  int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s >= n_stars) return;
+  const qlp_bls_star_grid g = grid[s];
+  const int64_t nf = (g.status == 0) ? g.n_freq : 0;
+  const double Q = dmul(prm.qmin_fac, g.c_q);
+  int64_t prev_lo = nf;
+  for (int c = 0; c < kNumClasses; ++c) {
+    int cap = class_nbcap(c);
+    int64_t lo = 0, hi = nf;  // answer in [0, nf]
+    if (force_path == 2 && c < 3) lo = nf;       // test hook: push everything to the 32-column class
+    else if (force_path == 3 && c < 8) lo = nf;  // test hook: one column per CTA for everything
+    else {
+      while (lo < hi) {
+        int64_t mid = lo + ((hi - lo) >> 1);
+        double f; int32_t nb;
+        freq_of_k(g.u0, g.h, Q, (double)prm.noverlap, mid, f, nb);
+        if (nb <= cap) hi = mid; else lo = mid + 1;
+      }
+    }
+    if (lo > prev_lo) lo = prev_lo;
+    kb[s * kNumClasses + c] = lo;
+    int64_t span = prev_lo - lo;
+    int cols = class_cols(c);
+    cnt[c * n_stars + s] = (span + cols - 1) / cols;
+    prev_lo = lo;
+  }
+}
+
+// One CTA per class: exclusive scan of cnt[c][0..S) -> off[c][0..S].
+__global__ void __launch_bounds__(1024) tile_scan_kernel(int64_t n_stars, const int64_t* __restrict__ cnt,
+                                                         int64_t* __restrict__ off) {
+  const int c = blockIdx.x;
+  const int64_t* in = cnt + (int64_t)c * n_stars;
+  int64_t* out = off + (int64_t)c * (n_stars + 1);
+  __shared__ int64_t warp_sum[32];
+  __shared__ int64_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int64_t base = 0; base < n_stars; base += blockDim.x) {
+    int64_t i = base + threadIdx.x;
+    int64_t v = (i < n_stars) ? in[i] : 0;
+    int64_t x = v;
+    for (int o = 1; o < 32; o <<= 1) {
+      int64_t y = __shfl_up_sync(0xffffffffu, x, o);
+      if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_sum[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+      int64_t w = warp_sum[lane];
+      for (int o = 1; o < 32; o <<= 1) {
+        int64_t y = __shfl_up_sync(0xffffffffu, w, o);
+        if (lane >= o) w += y;
+      }
+      warp_sum[lane] = w;
+    }
+    __syncthreads();
+    int64_t prefix = carry + (wid > 0 ? warp_sum[wid - 1] : 0) + x - v;
+    if (i < n_stars) out[i] = prefix;
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) carry = prefix + v;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[n_stars] = carry;
+}
+
+// ---- the fused kernel ---------------------------------------------------------------------------
+struct TileInfo {
+  int64_t k0, pt_begin, n_pts, out_base;
+  double u0, h, Q;
+  float inv_w, inv_s;
+  int32_t ncols, nb_tile;
+  int32_t valid;
+};
+
+template <int MW>
+__global__ void __launch_bounds__(kThreads) foldscan_kernel(
+    Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
+    const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
+    const int64_t* __restrict__ freq_ptr, const int64_t* __restrict__ tile_off, const int64_t* __restrict__ kb,
+    unsigned long long* __restrict__ counter, float* __restrict__ sr, uint32_t* __restrict__ best) {
+  extern __shared__ __align__(16) uint32_t hist[];
+  __shared__ TileInfo ti;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int ctot = class_cols(cls);         // columns per CTA
+  const int stride = 2 * ctot;              // words per histogram row: [W x ctot][S x ctot]
+  const int cw = ctot < 32 ? ctot : 32;     // columns per warp
+  const int hpw = 32 / cw;                  // points per warp iteration
+  const int groups = ctot / cw;             // column groups (2 for 64 columns, else 1)
+  const int grp = warp % groups, slice = warp / groups, nslices = kWarps / groups;
+  const int col = grp * cw + (lane % cw);   // this lane's column in the fold phase
+  const int hsub = lane / cw;
+  const double dno = (double)prm.noverlap;
+  const int64_t n_tiles = tile_off[n_stars];
+
+  for (;;) {
+    __syncthreads();  // previous tile fully written before ti / hist are reused
+    if (tid == 0) {
+      int64_t tile = (int64_t)atomicAdd(counter, 1ull);
+      TileInfo x;
+      x.valid = tile < n_tiles;
+      if (x.valid) {
+        int64_t lo = 0, hi = n_stars - 1;  // last s with tile_off[s] <= tile
+        while (lo < hi) {
+          int64_t mid = lo + ((hi - lo + 1) >> 1);
+          if (tile_off[mid] <= tile) lo = mid; else hi = mid - 1;
+        }
+        const int64_t s = lo;
+        const qlp_bls_star_grid g = grid[s];
+        const StarPrep sp = prep[s];
+        const int64_t k_lo = kb[s * kNumClasses + cls];
+        const int64_t k_hi = (cls == 0) ? g.n_freq : kb[s * kNumClasses + cls - 1];
+        x.k0 = k_lo + (tile - tile_off[s]) * ctot;
+        int64_t rem = k_hi - x.k0;
+        x.ncols = rem < ctot ? (int32_t)rem : ctot;
+        x.pt_begin = row_ptr[s];
+        x.n_pts = row_ptr[s + 1] - row_ptr[s];
+        x.out_base = freq_ptr[s];
+        x.u0 = g.u0; x.h = g.h; x.Q = dmul(prm.qmin_fac, g.c_q);
+        x.inv_w = sp.inv_w; x.inv_s = sp.inv_s;
+        double f; int32_t nb;
+        freq_of_k(x.u0, x.h, x.Q, dno, x.k0, f, nb);
+        x.nb_tile = nb;
+      }
+      ti = x;
+    }
+    __syncthreads();
+    if (!ti.valid) break;
+    const int nb_tile = ti.nb_tile;
+    // zero the histograms of this tile
+    {
+      const int words = nb_tile * stride;
+      uint4* h4 = reinterpret_cast<uint4*>(hist);
+      for (int i = tid; i < (words >> 2); i += kThreads) h4[i] = make_uint4(0u, 0u, 0u, 0u);
+      for (int i = (words & ~3) + tid; i < words; i += kThreads) hist[i] = 0u;
+    }
+    // ---- S2: fold ----
+    {
+      double f = 0.0; int32_t nbk = 1;
+      const bool col_on = col < ti.ncols;
+      if (col_on) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f, nbk);
+      const double dnb = (double)nbk, K = (dnb + 1.0) * QLP_TWO52;
+      __syncthreads();
+      const int4* p4 = reinterpret_cast<const int4*>(pts + ti.pt_begin);
+      const int64_t n = ti.n_pts;
+      const int64_t step = (int64_t)nslices * hpw;
+      uint32_t* hcol = hist + col;
+      if (col_on) {
+#pragma unroll 4
+        for (int64_t i = (int64_t)slice * hpw + hsub; i < n; i += step) {
+          const int4 v = __ldg(p4 + i);
+          const double tau = __hiloint2double(v.y, v.x);
+          const int32_t b = bin_of(f, tau, dnb, K);
+          uint32_t* cell = hcol + b * stride;
+          atomicAdd(cell, (uint32_t)v.z);
+          atomicAdd(cell + ctot, (uint32_t)v.w);
+        }
+      }
+    }
+    __syncthreads();
+    // ---- S3: box scan, in place ----
+    const int tpc = kThreads / ctot;  // threads per column
+    const int scol = tid % ctot, seg = tid / ctot;
+    float bnum = 0.f, bden = 1.f;
+    int bm = prm.min_width, bj = 0;
+    const bool scol_on = scol < ti.ncols;
+    if (scol_on) {
+      double f; int32_t nbk;
+      freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, f, nbk);
+      const int per = (nbk + tpc - 1) / tpc;
+      const int ja = seg * per;
+      const int jb = min(nbk, ja + per);
+      const uint32_t* hc = hist + scol;
+      const float inv_w = ti.inv_w;
+      const uint32_t wmask = prm.wmask;
+      if (ja < jb) {
+        float ww[MW], ss[MW];
+#pragma unroll
+        for (int l = 0; l < MW - 1; ++l) {
+          int e = ja + l;
+          if (e >= nbk) e -= nbk;
+          ww[l] = (float)hc[e * stride] * inv_w;
+          ss[l] = (float)(int32_t)hc[e * stride + ctot];
+        }
+        ww[MW - 1] = 0.f; ss[MW - 1] = 0.f;
+        for (int j0 = ja; j0 < jb; j0 += MW) {
+#pragma unroll
+          for (int jj = 0; jj < MW; ++jj) {
+            const int j = j0 + jj;
+            if (j < jb) {
+              int e = j + MW - 1;
+              if (e >= nbk) e -= nbk;
+              ww[(jj + MW - 1) % MW] = (float)hc[e * stride] * inv_w;
+              ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * stride + ctot];
+              float r = ww[jj % MW], sm = ss[jj % MW];
+#pragma unroll
+              for (int m = 2; m <= MW; ++m) {
+                r += ww[(jj + m - 1) % MW];
+                sm += ss[(jj + m - 1) % MW];
+                if ((wmask >> m) & 1u) {
+                  const float d = fmaf(-r, r, r);  // r (1 - r)
+                  const float num = sm * sm;
+                  const float lhs = num * bden, rhs = bnum * d;
+                  if (d > 0.f && (lhs > rhs || (lhs == rhs && m < bm))) { bnum = num; bden = d; bm = m; bj = j; }
+                }
+              }
+              if (wmask & 2u) {  // width 1 (not on the paper's ladder; kept for completeness)
+                const float r1 = ww[jj % MW], s1 = ss[jj % MW];
+                const float d = fmaf(-r1, r1, r1), num = s1 * s1;
+                const float lhs = num * bden, rhs = bnum * d;
+                if (d > 0.f && (lhs > rhs || (lhs == rhs && 1 < bm))) { bnum = num; bden = d; bm = 1; bj = j; }
+              }
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();  // all reads of hist done: reuse it as reduction scratch
+    {
+      float* cnum = reinterpret_cast<float*>(hist);
+      float* cden = cnum + kThreads;
+      uint32_t* cidx = hist + 2 * kThreads;
+      cnum[tid] = bnum; cden[tid] = bden; cidx[tid] = ((uint32_t)bm << 24) | (uint32_t)bj;
+      __syncthreads();
+      if (seg == 0 && scol_on) {
+        for (int g2 = 1; g2 < tpc; ++g2) {
+          const int o = g2 * ctot + scol;
+          const float num = cnum[o], d = cden[o];
+          const uint32_t idx = cidx[o];
+          const int m = (int)(idx >> 24);
+          const float lhs = num * bden, rhs = bnum * d;
+          // later segments hold larger j: they win only if strictly better, or equal with smaller m
+          if (lhs > rhs || (lhs == rhs && num > 0.f && m < bm)) { bnum = num; bden = d; bm = m; bj = (int)(idx & 0xffffffu); }
+        }
+        const int64_t o = ti.out_base + ti.k0 + scol;
+        sr[o] = (bnum / bden) * ti.inv_s * ti.inv_s;
+        best[o] = ((uint32_t)bm << 24) | (uint32_t)bj;
+      }
+    }
+  }
+}
+
+}  // namespace qlp

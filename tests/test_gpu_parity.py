@@ -1,0 +1,282 @@
+"""GPU-vs-oracle parity (run with -m gpu on a B200).  Every comparison goes through the C ABI
+(paper_2302_01293_b200.bls -> libqlp_bls.so) on one side and oracle/ on the other, on the same
+seeded synthetic inputs (paper_2302_01293_b200.synth).
+
+Acceptance (BASELINE.json north_star):
+  * grid descriptors, freq_ptr, f_k, nb_k and bin indices: bit-exact;
+  * |SR_gpu - SR_oracle| <= 1e-4 * max_f SR_oracle per star;
+  * best (m, j) and peak frequency compared only where the runner-up is more than that tolerance away.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SR_RTOL = 1e-4  # of the per-star peak (north_star)
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2302_01293_b200 import build, bls
+    build.build()
+    return bls
+
+
+@pytest.fixture(scope="module")
+def ctx(gpu):
+    c = gpu.QlpBls()
+    yield c
+    c.close()
+
+
+def _oracle_grids(orc, cfg, batch):
+    gs = np.zeros(batch.n_stars, dtype=orc.GRID_DTYPE)
+    for s in range(batch.n_stars):
+        t, _, _ = batch.star(s)
+        gs[s] = orc.grid(cfg, t, float(batch.rho[s]))
+    return gs
+
+
+GRID_FIELDS = ["t_ref", "baseline", "p_min", "p_max", "c_q", "u0", "h", "n_freq", "nb_max", "status"]
+
+
+def _assert_grid_equal(g_gpu, g_orc):
+    for f in GRID_FIELDS:
+        a, b = g_gpu[f], g_orc[f]
+        if a.dtype.kind == "f":
+            assert np.array_equal(a.view(np.int64), b.view(np.int64)), f"grid field {f} not bit-exact"
+        else:
+            assert np.array_equal(a, b), f"grid field {f} differs"
+
+
+def _batches():
+    from paper_2302_01293_b200 import synth
+    return {
+        "c1": synth.make_batch(1),
+        "c2": synth.make_batch(2, n_stars=6),
+        "c3": synth.make_batch(3, n_stars=4),
+        "c4": synth.make_batch(4, n_stars=2),
+        "c5": synth.make_batch(5, star_ids=np.arange(40)),
+    }
+
+
+@pytest.fixture(scope="module")
+def batches():
+    return _batches()
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4", "c5"])
+def test_grid_bit_exact(gpu, ctx, orc, cfg, batches, name):
+    b = batches[name]
+    dev = gpu.upload(b)
+    grid, freq_ptr, tf, tb = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    g = gpu.grid_to_numpy(grid)
+    go = _oracle_grids(orc, cfg, b)
+    _assert_grid_equal(g, go)
+    fp = freq_ptr.cpu().numpy()
+    assert np.array_equal(fp, np.concatenate([[0], np.cumsum(go["n_freq"])]))
+    assert tf == int(go["n_freq"].sum())
+    # f_k, nb_k bit-exact on the first and last star, whole grid
+    total_bins = 0
+    for s in range(b.n_stars):
+        f_o, nb_o = orc.freqs(cfg, go[s])
+        total_bins += int(nb_o.sum())
+        if s in (0, b.n_stars - 1):
+            f_g, nb_g = ctx.debug_freqs(grid, s, 0, int(go[s]["n_freq"]))
+            assert np.array_equal(f_g.cpu().numpy().view(np.int64), f_o.view(np.int64))
+            assert np.array_equal(nb_g.cpu().numpy(), nb_o)
+    assert tb == total_bins
+
+
+def test_grid_edge_cases(gpu, ctx, orc, cfg):
+    from paper_2302_01293_b200 import synth
+    cad = 0.02
+    mk = lambda t: (np.asarray(t, dtype=np.float64), np.zeros(len(t)), np.ones(len(t)))
+    stars = [
+        mk(np.arange(0, 50, cad)),                                                  # no gap -> L/2
+        mk(np.concatenate([np.arange(0, 20, cad), np.arange(21, 60, cad)])),        # 1-d gap only
+        mk(np.concatenate([np.arange(0, 20, cad), np.arange(50, 110, cad)])),       # 30-d gap -> longest side
+        mk(np.concatenate([np.arange(0, 20, cad), [19.98 + 27.4], 19.98 + 27.4 + np.arange(1, 500) * cad])),
+        mk(np.concatenate([np.arange(0, 20, cad), 19.98 + 27.4 + cad + np.arange(0, 500) * cad])),
+        mk([]),                                                                      # empty star
+        mk([5.0]),                                                                   # one point
+        mk([1.0, 1.0 + 1e-9]),                                                       # P_max <= P_min
+        mk(np.arange(0, 30, cad)),
+    ]
+    rho = np.array([1.0, 0.3, 2.5, 1.0, 1.0, 1.0, 1.0, 1.0, np.nan])
+    b = synth.from_arrays(stars, rho=rho)
+    dev = gpu.upload(b)
+    grid, freq_ptr, tf, tb = ctx.grid(dev[0], dev[1], dev[4], None)
+    g = gpu.grid_to_numpy(grid)
+    go = _oracle_grids(orc, cfg, b)
+    _assert_grid_equal(g, go)
+    assert list(g["status"][5:8]) == [1, 1, 3]
+    assert g["n_freq"][5] == 0 and g["n_freq"][7] == 0
+
+
+def test_empty_batch(gpu, ctx):
+    import torch
+    z = torch.zeros(1, dtype=torch.int64, device="cuda")
+    e = torch.zeros(0, dtype=torch.float64, device="cuda")
+    grid, freq_ptr, tf, tb = ctx.grid(z, e, e, e)
+    assert tf == 0 and tb == 0 and freq_ptr.cpu().tolist() == [0]
+    sr, best = ctx.spectrum(z, e, e, e, grid, freq_ptr, 0)
+    assert sr.numel() == 0
+
+
+@pytest.mark.parametrize("name", ["c1", "c3", "c4", "c5"])
+def test_bins_bit_exact(gpu, ctx, orc, cfg, batches, name):
+    b = batches[name]
+    dev = gpu.upload(b)
+    grid, _, _, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    go = _oracle_grids(orc, cfg, b)
+    rng = np.random.default_rng(7)
+    for s in [0, b.n_stars - 1]:
+        nf = int(go[s]["n_freq"])
+        if nf == 0:
+            continue
+        t, _, _ = b.star(s)
+        tau = t - go[s]["t_ref"]
+        ks = sorted({0, 1, nf // 2, nf - 1, *rng.integers(0, nf, 12).tolist()})
+        for k in ks:
+            f_o, nb_o = orc.freqs(cfg, go[s], k, k + 1)
+            bo = orc.bins(float(f_o[0]), int(nb_o[0]), tau)
+            bg = ctx.debug_bins(dev[0], dev[1], grid, s, k, t.size).cpu().numpy()
+            assert np.array_equal(bg, bo), (name, s, k, int((bg != bo).sum()))
+            assert bo.min() >= 0 and bo.max() < nb_o[0]
+
+
+def test_prep_matches(gpu, ctx, orc, cfg, batches):
+    b = batches["c2"]
+    dev = gpu.upload(b)
+    grid, _, _, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    go = _oracle_grids(orc, cfg, b)
+    for s in [0, b.n_stars - 1]:
+        t, y, dy = b.star(s)
+        tau_o, w_o, wy_o = orc.prep(t, y, dy, float(go[s]["t_ref"]))
+        tau, w, wy = ctx.debug_prep(dev[0], dev[1], dev[2], dev[3], grid, s, t.size)
+        assert np.array_equal(tau.cpu().numpy(), tau_o)
+        assert np.allclose(w.cpu().numpy(), w_o, rtol=1e-4, atol=0)
+        assert np.abs(wy.cpu().numpy() - wy_o).max() <= 1e-4 * np.abs(wy_o).max()
+
+
+def _compare_sr(sr_g, best_g, sr_o, m_o, j_o, label):
+    peak = float(sr_o.max()) if sr_o.size else 0.0
+    tol = SR_RTOL * peak
+    err = np.abs(sr_g.astype(np.float64) - sr_o)
+    assert err.max() <= tol, f"{label}: max |dSR| {err.max():.3e} > {tol:.3e}"
+    m_g = (best_g.astype(np.uint32) >> 24).astype(np.int64)
+    j_g = (best_g.astype(np.uint32) & 0xFFFFFF).astype(np.int64)
+    same = (m_g == m_o) & (j_g == j_o)
+    return err.max() / peak if peak > 0 else 0.0, float(same.mean()), m_g, j_g
+
+
+def _check_best_valid(orc, cfg, b, go, s, ks, m_g, j_g, sr_o, tol):
+    """Where (m, j) differs from the oracle's, the GPU's box must be as good within the tolerance."""
+    t, y, dy = b.star(s)
+    tau, w, wy = orc.prep(t, y, dy, float(go[s]["t_ref"]))
+    for k in ks:
+        f, nb = orc.freqs(cfg, go[s], int(k), int(k) + 1)
+        val = orc.sr_one(tau, w, wy, float(f[0]), int(nb[0]), np.array([m_g[k]]))  # best over j at the GPU's m
+        bo = orc.bins(float(f[0]), int(nb[0]), tau)
+        sel = ((bo - j_g[k]) % int(nb[0])) < m_g[k]
+        r, sv = w[sel].sum(), wy[sel].sum()
+        v = sv * sv / (r * (1 - r)) if 0 < r < 1 else 0.0
+        assert abs(v - sr_o[k]) <= 2 * tol, (s, k, v, sr_o[k], val)
+
+
+@pytest.mark.parametrize("name,path", [("c1", 0), ("c1", 2), ("c1", 3), ("c2", 0), ("c3", 0), ("c5", 0)])
+def test_sr_parity_full(gpu, ctx, orc, cfg, batches, name, path):
+    b = batches[name]
+    if name == "c5":  # keep the oracle within seconds: the cheapest 12 of the 40 stars
+        from paper_2302_01293_b200 import synth
+        order = np.argsort(np.diff(b.row_ptr))[:12]
+        b = synth.make_batch(5, star_ids=np.sort(order))
+    dev = gpu.upload(b)
+    ctx.debug_set_path(path)
+    try:
+        grid, freq_ptr, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, tf)
+        sr, best = sr.cpu().numpy(), best.cpu().numpy()
+    finally:
+        ctx.debug_set_path(0)
+    ob = orc.batch(cfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=0, want_snr=False)
+    fp = ob["freq_ptr"]
+    assert np.array_equal(fp, freq_ptr.cpu().numpy())
+    worst, agree = 0.0, []
+    for s in range(b.n_stars):
+        a, e = int(fp[s]), int(fp[s + 1])
+        if e == a:
+            continue
+        rel, same, m_g, j_g = _compare_sr(sr[a:e], best[a:e], ob["sr"][a:e], ob["m"][a:e], ob["j"][a:e], f"{name}[{s}]")
+        worst = max(worst, rel)
+        agree.append(same)
+        # argmax frequency identical wherever the top two oracle values differ by more than the tolerance
+        so = ob["sr"][a:e]
+        top = np.argsort(so)[-2:]
+        if so.size >= 2 and so[top[1]] - so[top[0]] > SR_RTOL * so[top[1]]:
+            assert int(np.argmax(sr[a:e])) == int(top[1])
+        bad = np.nonzero((m_g != ob["m"][a:e]) | (j_g != ob["j"][a:e]))[0]
+        _check_best_valid(orc, cfg, b, ob["grid"], s, bad[:20], m_g, j_g, so, SR_RTOL * so.max())
+    print(f"{name} path={path}: worst |dSR|/peak = {worst:.2e}, (m,j) identical on {np.mean(agree):.4f}")
+    assert np.mean(agree) > 0.98
+
+
+def test_sr_parity_sampled_long_baseline(gpu, ctx, orc, cfg, batches):
+    """Config 4 (13 sectors, 200 s): the oracle is evaluated one frequency at a time on a sample that
+    spans every tile class the star reaches."""
+    b = batches["c4"]
+    dev = gpu.upload(b)
+    grid, freq_ptr, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, tf)
+    sr, best, fp = sr.cpu().numpy(), best.cpu().numpy(), freq_ptr.cpu().numpy()
+    go = _oracle_grids(orc, cfg, b)
+    M = orc.widths(cfg)
+    rng = np.random.default_rng(11)
+    for s in range(b.n_stars):
+        nf = int(go[s]["n_freq"])
+        t, y, dy = b.star(s)
+        tau, w, wy = orc.prep(t, y, dy, float(go[s]["t_ref"]))
+        # uniform in sqrt(k) oversamples the low-frequency (large nb) end
+        ks = np.unique(np.concatenate([[0, 1, 2, nf - 1], (rng.random(60) ** 2 * nf).astype(np.int64),
+                                       rng.integers(0, nf, 30)]))
+        peak = float(sr[fp[s]:fp[s + 1]].max())
+        for k in ks:
+            f, nb = orc.freqs(cfg, go[s], int(k), int(k) + 1)
+            v, m, j, _, _ = orc.sr_one(tau, w, wy, float(f[0]), int(nb[0]), M)
+            g = float(sr[fp[s] + k])
+            assert abs(g - v) <= SR_RTOL * peak, (s, int(k), int(nb[0]), g, v)
+    # the sample must have reached the wide classes (nb > 880)
+    assert go["nb_max"].max() > 880
+
+
+def test_constant_and_degenerate_light_curves(gpu, ctx, orc, cfg):
+    from paper_2302_01293_b200 import synth
+    t = synth.sector_times(0, 1800.0)
+    rng = np.random.default_rng(3)
+    stars = [
+        (t, np.full(t.size, 1.234), np.full(t.size, 1e-3)),          # constant -> SR == 0 everywhere
+        (t, rng.standard_normal(t.size) * 1e-3 + 5.0, np.full(t.size, 1e-3)),  # large offset
+        (t[:2], np.array([0.0, 1.0]), np.array([1.0, 1.0])),           # two points (P_max <= P_min)
+        (np.array([]), np.array([]), np.array([])),
+        (t, rng.standard_normal(t.size) * 1e3, np.full(t.size, 1e3)),  # other flux units: scale invariance
+    ]
+    b = synth.from_arrays(stars)
+    dev = gpu.upload(b)
+    grid, freq_ptr, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, tf)
+    snr, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, sr, best)
+    sr, best, fp, snr = sr.cpu().numpy(), best.cpu().numpy(), freq_ptr.cpu().numpy(), snr.cpu().numpy()
+    pk = gpu.peaks_to_numpy(peaks, ctx.top_k)
+    assert np.all(sr[fp[0]:fp[1]] == 0.0)
+    assert np.all((best[fp[0]:fp[1]].astype(np.uint32) >> 24) == 3) and np.all((best[fp[0]:fp[1]] & 0xFFFFFF) == 0)
+    assert np.all(snr[fp[0]:fp[1]] == 0.0)
+    assert fp[3] == fp[2] and fp[4] == fp[3]
+    assert np.all(pk[2]["k"] == -1) and np.all(pk[3]["status"] == 1)
+    ob = orc.batch(cfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=0, want_snr=False)
+    for s in (1, 4):
+        so = ob["sr"][fp[s]:fp[s + 1]]
+        assert np.abs(sr[fp[s]:fp[s + 1]] - so).max() <= SR_RTOL * so.max()
