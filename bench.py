@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the QLP BLS hot path (S0..S4) on synthetic TESS-shaped light curves.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C] [--stars S]
+
+One "step" = one pass of the whole hot path (grid -> prep -> fold+box-scan -> S/N + peaks) over one
+batch.  Default workload = BASELINE.json configs[1] ("config 2": 1,000 stars, one sector at 200 s
+cadence, ~11.4k points and ~4.5k-10k frequencies per star).  Prints ONE JSON line (rank 0).
+
+  value     : point x frequency BLS evaluations per second, whole job, inputs resident in HBM
+  e2e       : the same metric through qlp_bls_search_host with pinned HOST buffers (H2D + D2H inside)
+  roofline  : fold+box-scan launches, CUDA-event timed inside the timed region, against the
+              shared-memory-atomic issue ceiling derived in DESIGN.md ("bound": "alu")
+  cpu_baseline : oracle/ timed on this box's host cores on a bounded sample (N=1, rank 0 only)
+
+`--impl reference` times the oracle (the only reference that exists for this paper) on the host.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "bls_point_frequency_evals_per_s"
+UNIT = "evals/s"
+# per evaluation the fold needs 2 shared-memory integer atomic lanes and 4 FP64
+# lanes; measured ceilings on B200 (profiles/ubench_r1.txt): ATOMS.ADD lanes/clk/SM and FP64
+# lanes/clk/SM.  The binding one is the atomic path.
+ATOMS_LANES_PER_CLK_SM = 16.0
+FP64_LANES_PER_CLK_SM = 64.0
+N_SM = 148
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def fold_peak_evals_per_s(sm_mhz: float) -> float:
+    per_clk_sm = min(ATOMS_LANES_PER_CLK_SM / 2.0, FP64_LANES_PER_CLK_SM / 4.0)
+    return N_SM * sm_mhz * 1e6 * per_clk_sm
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(config: int, n_stars: int, rank: int):
+    """Seeded synthetic batch; rank r takes star ids [r*n, (r+1)*n)."""
+    from paper_2302_01293_b200 import synth
+    ids = np.arange(rank * n_stars, (rank + 1) * n_stars, dtype=np.int64)
+    return synth.make_batch(config, star_ids=ids)
+
+
+def oracle_evals(orc, cfg, batch):
+    """Fold evaluations (points x frequencies) the oracle performs on this batch."""
+    tot = 0
+    for s in range(batch.n_stars):
+        t, _, _ = batch.star(s)
+        g = orc.grid(cfg, t, float(batch.rho[s]))
+        tot += int(g["n_freq"]) * t.size
+    return tot
+
+
+def time_oracle(batch, n_stars: int, threads: int):
+    """Run the oracle as it stands (OpenMP over stars) on the first n_stars -> (seconds, evals)."""
+    from oracle import oracle as orc
+    from paper_2302_01293_b200 import synth
+    cfg = orc.default_config()
+    sub = synth.from_arrays([batch.star(s) for s in range(n_stars)], rho=batch.rho[:n_stars])
+    ev = oracle_evals(orc, cfg, sub)
+    t0 = time.perf_counter()
+    orc.batch(cfg, sub.row_ptr, sub.t, sub.y, sub.dy, sub.rho, K=3, want_snr=True, threads=threads)
+    return time.perf_counter() - t0, ev
+
+
+def cpu_baseline(batch, budget_s: float = 15.0):
+    cores = os.cpu_count() or 1
+    from oracle import oracle as orc
+    orc.build()
+    n0 = min(batch.n_stars, cores)
+    dt0, ev0 = time_oracle(batch, n0, cores)
+    n1 = int(min(batch.n_stars, max(n0, n0 * budget_s / max(dt0, 1e-3))))
+    if n1 > n0:
+        dt, ev = time_oracle(batch, n1, cores)
+    else:
+        dt, ev, n1 = dt0, ev0, n0
+    return {"value": ev / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n1} stars of the workload, whole path (grid+SR+S/N+peaks), {dt:.1f} s",
+            "stars_per_s": n1 / dt}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import oracle as orc
+    orc.build()
+    cores = os.cpu_count() or 1
+    n = max(1, min(args.stars, 2 * cores))
+    batch = make_workload(args.config, n, 0)
+    for _ in range(args.warmup):
+        time_oracle(batch, min(n, cores), cores)
+    tot_t, tot_ev = 0.0, 0
+    for _ in range(args.steps):
+        dt, ev = time_oracle(batch, n, cores)
+        tot_t += dt; tot_ev += ev
+    val = tot_ev / tot_t
+    out = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+           "config": {"workload": f"config{args.config}: {n}-star sample of BASELINE.json configs[{args.config - 1}]"},
+           "stars_per_s": n * args.steps / tot_t,
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                            "sample": f"{n} stars per step, {args.steps} steps"},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2302_01293_b200 import build, bls
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the QLP BLS path has no CPU fallback)")
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.set_device(local)
+    ctx = bls.QlpBls(device=local, top_k=3)
+    # stars are independent: each rank searches its own shard, no data-path collective
+    batch = make_workload(args.config, args.stars, rank)
+    dev = bls.upload(batch, f"cuda:{local}")
+    row_ptr, t, y, dy, rho, rstar = dev
+    S = batch.n_stars
+
+    def step():
+        grid, freq_ptr, tf, _ = ctx.grid(row_ptr, t, rho, rstar)
+        sr, best = ctx.spectrum(row_ptr, t, y, dy, grid, freq_ptr, tf)
+        _, peaks = ctx.snr(row_ptr, t, y, dy, grid, freq_ptr, sr, best, want_snr=False)
+        return grid, peaks, tf
+
+    grid, peaks, tf = step()
+    g = bls.grid_to_numpy(grid)
+    evals = int((g["n_freq"] * np.diff(batch.row_ptr)).sum())
+    for _ in range(max(args.warmup - 1, 0)):
+        step()
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    ctx.fold_timing(True)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    ms = e0.elapsed_time(e1)
+    n_timed, fold_ms = ctx.fold_elapsed_ms()
+    ctx.fold_timing(False)
+
+    # end to end through the host-buffer API: pinned host inputs, H2D and D2H inside the timed region
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    h = [pin(batch.row_ptr), pin(batch.t), pin(batch.y), pin(batch.dy), pin(batch.rho)]
+    ctx.search_host(*h)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        pk_host, _, _ = ctx.search_host(*h)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    h2d = int(sum(a.nbytes for a in h))
+    d2h = int(pk_host.nbytes)
+
+    tvals = torch.tensor([ms, e2e_s * 1e3, float(evals), float(S)], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        mx = tvals.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = tvals.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        ms, e2e_ms, evals_all, stars_all = float(mx[0]), float(mx[1]), float(sm[2]), float(sm[3])
+    else:
+        e2e_ms, evals_all, stars_all = e2e_s * 1e3, float(evals), float(S)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks_info, src = _peaks()
+    sm_max = float(peaks_info.get("sm_max_mhz", 1965.0))
+    fold_per_launch_s = (fold_ms / max(n_timed, 1)) * 1e-3
+    achieved = evals / fold_per_launch_s if fold_per_launch_s > 0 else 0.0
+    peak = fold_peak_evals_per_s(sm_max)
+    out = {
+        "metric": METRIC, "value": evals_all * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64 phase / int32 fixed-point accumulators / f32 box scan",
+        "data": "synthetic",
+        "config": {"workload": f"config{args.config}: BASELINE.json configs[{args.config - 1}], {S} stars per GPU, "
+                               f"{int(batch.n_points)} points, {int(tf)} frequencies",
+                   "l2": "inputs larger than L2 (no flush needed)" if batch.n_points * 24 > 126e6 else
+                         "inputs smaller than L2", "parallelism": f"stars sharded over {world} GPU(s), no collective"},
+        "stars_per_s": stars_all * args.steps / (ms * 1e-3),
+        "clocks": clocks,
+        "e2e": {"value": evals_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "stars_per_s": stars_all * args.steps / (e2e_ms * 1e-3)},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
+                     "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",
+                     "frac": achieved / peak if peak > 0 else None, "traffic": None,
+                     "share_of_step": fold_ms / max(n_timed, 1) / (ms / args.steps),
+                     "peak_source": f"148 SMs x {sm_max:.0f} MHz ({src}) x min(ATOMS lanes/2, FP64 lanes/4) per clk "
+                                    "(profiles/ubench_r1.txt; DESIGN.md Roofline)"},
+    }
+    if world == 1 and not args.no_cpu:
+        out["cpu_baseline"] = cpu_baseline(batch)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[config-1]")
+    ap.add_argument("--stars", type=int, default=1000, help="stars per GPU")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -154,6 +154,15 @@ const char* qlp_bls_strerror(int code);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 int64_t qlp_bls_launch_count(const qlp_bls_ctx* ctx);
 
+/* CUDA-event timing of the fold/scan launches inside qlp_bls_spectrum (the dominant kernel; used by
+ * bench.py for the roofline figure).  enable != 0 starts recording one event pair per spectrum call
+ * on the call's stream (a ring of 256) and resets the call count. */
+int qlp_bls_fold_timing(qlp_bls_ctx* ctx, int32_t enable);
+
+/* Waits for the recorded events; *n_calls = spectrum calls timed (<= 256), *total_ms = summed device
+ * time of their fold/scan launches. */
+int qlp_bls_fold_elapsed_ms(qlp_bls_ctx* ctx, int32_t* n_calls /*host*/, double* total_ms /*host*/);
+
 /* The duration ladder in fine bins (O1.9): writes up to cap widths to m (host),
  * returns their number. */
 int qlp_bls_widths(const qlp_bls_ctx* ctx, int32_t* m /*host*/, int32_t cap);

@@ -36,7 +36,7 @@ PEAK_DTYPE = np.dtype([("k", "i8"), ("freq", "f8"), ("period", "f8"), ("t0", "f8
 
 EXPORTS = ["qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
-           "qlp_bls_widths", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
+           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
 
 _lib = None
@@ -68,6 +68,8 @@ def load_library():
         L.qlp_bls_debug_bins.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp]
         L.qlp_bls_debug_prep.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp]
         L.qlp_bls_debug_set_path.argtypes = [vp, i32]
+        L.qlp_bls_fold_timing.argtypes = [vp, i32]
+        L.qlp_bls_fold_elapsed_ms.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -132,6 +134,15 @@ class QlpBls:
         m = np.zeros(32, dtype=np.int32)
         n = self.lib.qlp_bls_widths(self._h, m.ctypes.data_as(C.c_void_p), 32)
         return m[:n].copy()
+
+    def fold_timing(self, enable: bool):
+        _check(self.lib.qlp_bls_fold_timing(self._h, 1 if enable else 0), "qlp_bls_fold_timing")
+
+    def fold_elapsed_ms(self):
+        """-> (number of spectrum calls timed, summed device ms of their fold/scan launches)."""
+        n, ms = C.c_int32(), C.c_double()
+        _check(self.lib.qlp_bls_fold_elapsed_ms(self._h, C.byref(n), C.byref(ms)), "qlp_bls_fold_elapsed_ms")
+        return int(n.value), float(ms.value)
 
     def debug_set_path(self, path: int):
         _check(self.lib.qlp_bls_debug_set_path(self._h, path), "qlp_bls_debug_set_path")

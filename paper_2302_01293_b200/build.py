@@ -13,6 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libqlp_bls.so")
+UBENCH = os.path.join(_HERE, "qlp_ubench")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
 
@@ -36,6 +37,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.run(cmd, check=True)
+    src = os.path.join(CSRC, "ubench.cu")
+    if force or not os.path.exists(UBENCH) or os.path.getmtime(UBENCH) < os.path.getmtime(src):
+        nvcc = os.environ.get("NVCC", "nvcc")
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                        "-cudart", "static", "-o", UBENCH, src], check=True)
     return LIB
 
 

@@ -47,6 +47,12 @@ struct qlp_bls_ctx {
   // cache of the last grid call: lets spectrum/snr size the point workspace without a sync
   const int64_t* last_row_ptr = nullptr;
   int64_t last_n_stars = -1, last_n_points = -1;
+  // optional per-call CUDA-event timing of the fold/scan launches (bench.py's roofline figure)
+  static const int kRing = 256;
+  bool timing = false;
+  cudaEvent_t ev0[kRing], ev1[kRing];
+  bool ev_ready = false;
+  int64_t ev_calls = 0;
 };
 
 #define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { cudaGetLastError(); return QLP_BLS_ECUDA; } } while (0)
@@ -126,7 +132,7 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
   }
   ctx->n_sm = n_sm;
-  const int max_smem = 227 * 1024;
+  const int max_smem = 64 * 440 * 8;  // largest class: 225,280 B (+ static) <= 227 KB
   if (cudaFuncSetAttribute(foldscan_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
       cudaFuncSetAttribute(foldscan_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
       cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
@@ -148,6 +154,8 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks};
   for (DevBuf* b : bufs) b->release();
   if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
+  if (ctx->ev_ready)
+    for (int i = 0; i < qlp_bls_ctx::kRing; ++i) { cudaEventDestroy(ctx->ev0[i]); cudaEventDestroy(ctx->ev1[i]); }
   delete ctx;
   return QLP_BLS_OK;
 }
@@ -171,6 +179,37 @@ extern "C" int qlp_bls_widths(const qlp_bls_ctx* ctx, int32_t* m, int32_t cap) {
   int n = ctx->n_widths < cap ? ctx->n_widths : cap;
   for (int i = 0; i < n; ++i) m[i] = ctx->widths[i];
   return ctx->n_widths;
+}
+
+extern "C" int qlp_bls_fold_timing(qlp_bls_ctx* ctx, int32_t enable) {
+  if (!ctx) return QLP_BLS_EINVAL;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  if (enable && !ctx->ev_ready) {
+    for (int i = 0; i < qlp_bls_ctx::kRing; ++i) {
+      CUDA_TRY(cudaEventCreate(&ctx->ev0[i]));
+      CUDA_TRY(cudaEventCreate(&ctx->ev1[i]));
+    }
+    ctx->ev_ready = true;
+  }
+  ctx->timing = enable != 0;
+  ctx->ev_calls = 0;
+  return QLP_BLS_OK;
+}
+
+extern "C" int qlp_bls_fold_elapsed_ms(qlp_bls_ctx* ctx, int32_t* n_calls, double* total_ms) {
+  if (!ctx || !n_calls || !total_ms || !ctx->ev_ready) return QLP_BLS_EINVAL;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  int64_t n = ctx->ev_calls < qlp_bls_ctx::kRing ? ctx->ev_calls : qlp_bls_ctx::kRing;
+  double sum = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    float ms = 0.f;
+    CUDA_TRY(cudaEventSynchronize(ctx->ev1[i]));
+    CUDA_TRY(cudaEventElapsedTime(&ms, ctx->ev0[i], ctx->ev1[i]));
+    sum += ms;
+  }
+  *n_calls = (int32_t)n;
+  *total_ms = sum;
+  return QLP_BLS_OK;
 }
 
 extern "C" int qlp_bls_debug_set_path(qlp_bls_ctx* ctx, int32_t path) {
@@ -257,6 +296,8 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   QLP_TRY(launch_ok(ctx));
   tile_scan_kernel<<<kNumClasses, 1024, 0, st>>>(n_stars, cnt, off);
   QLP_TRY(launch_ok(ctx));
+  const int slot = (int)(ctx->ev_calls % qlp_bls_ctx::kRing);
+  if (ctx->timing) CUDA_TRY(cudaEventRecord(ctx->ev0[slot], st));
   for (int c = 0; c < kNumClasses; ++c) {
     const size_t smem = (size_t)class_cols(c) * class_nbcap(c) * 8;
     const int per_sm = (c == 0) ? 4 : (c == 1 ? 2 : 1);
@@ -272,6 +313,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
                                                       counters + c, sr, best);
     QLP_TRY(launch_ok(ctx));
   }
+  if (ctx->timing) { CUDA_TRY(cudaEventRecord(ctx->ev1[slot], st)); ctx->ev_calls++; }
   return QLP_BLS_OK;
 }
 
