@@ -36,8 +36,8 @@ UNIT = "evals/s"
 # per evaluation the fold needs 2 shared-memory integer atomic lanes and 4 FP64
 # lanes; measured ceilings on B200 (profiles/ubench_r1.txt): ATOMS.ADD lanes/clk/SM and FP64
 # lanes/clk/SM.  The binding one is the atomic path.
-ATOMS_LANES_PER_CLK_SM = 16.0
-FP64_LANES_PER_CLK_SM = 64.0
+ATOMS_LANES_PER_CLK_SM = 31.6
+FP64_LANES_PER_CLK_SM = 62.3
 N_SM = 148
 
 

@@ -132,9 +132,17 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
   }
   ctx->n_sm = n_sm;
-  const int max_smem = 64 * 440 * 8;  // largest class: 225,280 B (+ static) <= 227 KB
-  if (cudaFuncSetAttribute(foldscan_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(foldscan_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) != cudaSuccess ||
+  int max_smem = 0;  // largest class: 231,440 B (+ static) <= 227 KB
+  for (int c = 0; c < kNumClasses; ++c) max_smem = class_smem_bytes(c) > max_smem ? class_smem_bytes(c) : max_smem;
+  bool attr_ok = true;
+#define QLP_ATTR(CT_)                                                                                                \
+  attr_ok = attr_ok &&                                                                                               \
+            cudaFuncSetAttribute(foldscan_kernel<11, CT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
+                cudaSuccess &&                                                                                       \
+            cudaFuncSetAttribute(foldscan_kernel<16, CT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
+                cudaSuccess
+  QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
+  if (!attr_ok ||
       cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
   }
@@ -299,18 +307,25 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   const int slot = (int)(ctx->ev_calls % qlp_bls_ctx::kRing);
   if (ctx->timing) CUDA_TRY(cudaEventRecord(ctx->ev0[slot], st));
   for (int c = 0; c < kNumClasses; ++c) {
-    const size_t smem = (size_t)class_cols(c) * class_nbcap(c) * 8;
-    const int per_sm = (c == 0) ? 4 : (c == 1 ? 2 : 1);
+    const size_t smem = (size_t)class_smem_bytes(c);
+    const int per_sm = (c == 0) ? 3 : (c == 1 ? 2 : 1);
     const unsigned nblk = (unsigned)(ctx->n_sm * per_sm);
     const int64_t* off_c = off + (int64_t)c * (n_stars + 1);
-    if (ctx->prm.max_width <= 11)
-      foldscan_kernel<11><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,
-                                                      (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,
-                                                      counters + c, sr, best);
-    else
-      foldscan_kernel<16><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,
-                                                      (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,
-                                                      counters + c, sr, best);
+    const bool wide = ctx->prm.max_width > 11;
+#define QLP_LAUNCH(MW_, CT_)                                                                                          \
+  foldscan_kernel<MW_, CT_><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,    \
+                                                         (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,    \
+                                                         counters + c, sr, best)
+#define QLP_LAUNCH_MW(CT_) do { if (wide) QLP_LAUNCH(16, CT_); else QLP_LAUNCH(11, CT_); } while (0)
+    switch (class_cols(c)) {
+      case 64: QLP_LAUNCH_MW(64); break;
+      case 32: QLP_LAUNCH_MW(32); break;
+      case 16: QLP_LAUNCH_MW(16); break;
+      case 8: QLP_LAUNCH_MW(8); break;
+      case 4: QLP_LAUNCH_MW(4); break;
+      case 2: QLP_LAUNCH_MW(2); break;
+      default: QLP_LAUNCH_MW(1); break;
+    }
     QLP_TRY(launch_ok(ctx));
   }
   if (ctx->timing) { CUDA_TRY(cudaEventRecord(ctx->ev1[slot], st)); ctx->ev_calls++; }

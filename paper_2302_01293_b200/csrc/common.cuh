@@ -112,9 +112,15 @@ __host__ __device__ __forceinline__ int class_cols(int c) {
   return c <= 2 ? 64 : (32 >> (c - 3));
 }
 __host__ __device__ __forceinline__ int class_nbcap(int c) {
-  // shared memory = cols * nbcap * 8 bytes
-  const int caps[kNumClasses] = {110, 220, 440, 880, 1760, 3520, 7040, 14080, 24576};
+  // shared memory = cols * nbcap * 8 bytes of histograms + kStageBytes of point staging;
+  // class 0 fits 3 CTAs per SM, class 1 two, the others one.
+  const int caps[kNumClasses] = {116, 192, 420, 840, 1680, 3360, 6720, 13440, 24576};
   return caps[c];
+}
+constexpr int kChunk = 512;                                   // points per staged chunk
+constexpr int kStageBytes = 2 * kChunk * 16 + 16;             // two buffers + two mbarriers
+__host__ __device__ __forceinline__ int class_smem_bytes(int c) {
+  return class_cols(c) * class_nbcap(c) * 8 + kStageBytes;
 }
 
 }  // namespace qlp

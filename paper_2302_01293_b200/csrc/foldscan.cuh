@@ -94,7 +94,30 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int64_t n_stars, const 
   if (threadIdx.x == 0) out[n_stars] = carry;
 }
 
-// ---- the fused kernel ---------------------------------------------------------------------------
+// ---- TMA bulk-copy staging of the point stream (cp.async.bulk -> SASS UBLKCP) -----------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
 struct TileInfo {
   int64_t k0, pt_begin, n_pts, out_base;
   double u0, h, Q;
@@ -103,25 +126,40 @@ struct TileInfo {
   int32_t valid;
 };
 
-template <int MW>
-__global__ void __launch_bounds__(kThreads) foldscan_kernel(
+// ---- the fused kernel ---------------------------------------------------------------------------
+// MW = widest box (window registers), CTOT = columns per CTA of this class (compile time so that the
+// two atomics of one evaluation differ by an immediate offset and the row stride is a shift).
+template <int MW, int CTOT>
+__global__ void __launch_bounds__(kThreads, (CTOT == 64 ? 3 : 1)) foldscan_kernel(
     Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const int64_t* __restrict__ tile_off, const int64_t* __restrict__ kb,
     unsigned long long* __restrict__ counter, float* __restrict__ sr, uint32_t* __restrict__ best) {
-  extern __shared__ __align__(16) uint32_t hist[];
+  extern __shared__ __align__(16) unsigned char smem[];
+  Point* pbuf = reinterpret_cast<Point*>(smem);                       // [2][kChunk]
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem + 2 * kChunk * 16);  // [2]
+  uint32_t* hist = reinterpret_cast<uint32_t*>(smem + kStageBytes);   // [nb_tile][2 * CTOT]
   __shared__ TileInfo ti;
+  constexpr int STRIDE = 2 * CTOT;              // words per histogram row: [W x CTOT][S x CTOT]
+  constexpr int CW = CTOT < 32 ? CTOT : 32;     // columns per warp
+  constexpr int HPW = 32 / CW;                  // points per warp iteration
+  constexpr int GROUPS = CTOT / CW;             // column groups (2 for 64 columns, else 1)
+  constexpr int NSLICES = kWarps / GROUPS;
+  constexpr int STEP = NSLICES * HPW;           // points consumed per iteration by one column group
+  constexpr int ITERS = kChunk / STEP;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int ctot = class_cols(cls);         // columns per CTA
-  const int stride = 2 * ctot;              // words per histogram row: [W x ctot][S x ctot]
-  const int cw = ctot < 32 ? ctot : 32;     // columns per warp
-  const int hpw = 32 / cw;                  // points per warp iteration
-  const int groups = ctot / cw;             // column groups (2 for 64 columns, else 1)
-  const int grp = warp % groups, slice = warp / groups, nslices = kWarps / groups;
-  const int col = grp * cw + (lane % cw);   // this lane's column in the fold phase
-  const int hsub = lane / cw;
+  const int grp = warp % GROUPS, slice = warp / GROUPS;
+  const int col = grp * CW + (lane % CW);       // this lane's column in the fold phase
+  const int hsub = lane / CW;
   const double dno = (double)prm.noverlap;
   const int64_t n_tiles = tile_off[n_stars];
+  uint32_t use0 = 0, use1 = 0;                  // completed uses of each staging buffer (phase parity)
+  if (tid == 0) {
+    mbar_init(&mbar[0], 1);
+    mbar_init(&mbar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
 
   for (;;) {
     __syncthreads();  // previous tile fully written before ti / hist are reused
@@ -140,9 +178,9 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
         const StarPrep sp = prep[s];
         const int64_t k_lo = kb[s * kNumClasses + cls];
         const int64_t k_hi = (cls == 0) ? g.n_freq : kb[s * kNumClasses + cls - 1];
-        x.k0 = k_lo + (tile - tile_off[s]) * ctot;
+        x.k0 = k_lo + (tile - tile_off[s]) * CTOT;
         int64_t rem = k_hi - x.k0;
-        x.ncols = rem < ctot ? (int32_t)rem : ctot;
+        x.ncols = rem < CTOT ? (int32_t)rem : CTOT;
         x.pt_begin = row_ptr[s];
         x.n_pts = row_ptr[s + 1] - row_ptr[s];
         x.out_base = freq_ptr[s];
@@ -151,18 +189,32 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
         double f; int32_t nb;
         freq_of_k(x.u0, x.h, x.Q, dno, x.k0, f, nb);
         x.nb_tile = nb;
+        // start streaming the first two chunks of the star's points
+        const Point* src = pts + x.pt_begin;
+        const int64_t n = x.n_pts;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if (n > 0) {
+          const uint32_t b0 = (uint32_t)((n < kChunk ? n : kChunk) * 16);
+          mbar_expect_tx(&mbar[0], b0);
+          bulk_load(pbuf, src, b0, &mbar[0]);
+        }
+        if (n > kChunk) {
+          const int64_t r = n - kChunk;
+          const uint32_t b1 = (uint32_t)((r < kChunk ? r : kChunk) * 16);
+          mbar_expect_tx(&mbar[1], b1);
+          bulk_load(pbuf + kChunk, src + kChunk, b1, &mbar[1]);
+        }
       }
       ti = x;
     }
     __syncthreads();
     if (!ti.valid) break;
     const int nb_tile = ti.nb_tile;
-    // zero the histograms of this tile
-    {
-      const int words = nb_tile * stride;
+    {  // zero the histograms of this tile
+      const int words = nb_tile * STRIDE;  // multiple of 2; hist is 16-byte aligned
       uint4* h4 = reinterpret_cast<uint4*>(hist);
       for (int i = tid; i < (words >> 2); i += kThreads) h4[i] = make_uint4(0u, 0u, 0u, 0u);
-      for (int i = (words & ~3) + tid; i < words; i += kThreads) hist[i] = 0u;
+      if (tid < (words & 3)) hist[(words & ~3) + tid] = 0u;
     }
     // ---- S2: fold ----
     {
@@ -170,34 +222,58 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
       const bool col_on = col < ti.ncols;
       if (col_on) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f, nbk);
       const double dnb = (double)nbk, K = (dnb + 1.0) * QLP_TWO52;
-      __syncthreads();
-      const int4* p4 = reinterpret_cast<const int4*>(pts + ti.pt_begin);
       const int64_t n = ti.n_pts;
-      const int64_t step = (int64_t)nslices * hpw;
+      const Point* src = pts + ti.pt_begin;
+      const int64_t n_chunks = (n + kChunk - 1) / kChunk;
+      // a column that is switched off folds into its own (unused) cells with weight from the points;
+      // cheaper than predicating every atomic: its histogram is never scanned.
       uint32_t* hcol = hist + col;
-      if (col_on) {
-#pragma unroll 4
-        for (int64_t i = (int64_t)slice * hpw + hsub; i < n; i += step) {
-          const int4 v = __ldg(p4 + i);
+      __syncthreads();  // histograms zeroed
+      for (int64_t c = 0; c < n_chunks; ++c) {
+        const int b = (int)(c & 1);
+        Point* buf = pbuf + b * kChunk;
+        mbar_wait(&mbar[b], (b ? use1 : use0) & 1u);
+        if (b) ++use1; else ++use0;
+        const int64_t left = n - c * kChunk;
+        if (left < kChunk) {  // pad the tail with weightless points so that every chunk is full
+          for (int i = (int)left + tid; i < kChunk; i += kThreads) {
+            Point z; z.tau = 0.0; z.W = 0u; z.S = 0;
+            buf[i] = z;
+          }
+          __syncthreads();
+        }
+        const int4* p4 = reinterpret_cast<const int4*>(buf) + slice * HPW + hsub;
+#pragma unroll 8
+        for (int it = 0; it < ITERS; ++it) {
+          const int4 v = p4[it * STEP];
           const double tau = __hiloint2double(v.y, v.x);
-          const int32_t b = bin_of(f, tau, dnb, K);
-          uint32_t* cell = hcol + b * stride;
+          const int32_t bb = bin_of(f, tau, dnb, K);
+          uint32_t* cell = hcol + bb * STRIDE;
           atomicAdd(cell, (uint32_t)v.z);
-          atomicAdd(cell + ctot, (uint32_t)v.w);
+          atomicAdd(cell + CTOT, (uint32_t)v.w);
+        }
+        __syncthreads();  // everyone is done with this buffer
+        if (tid == 0 && c + 2 < n_chunks) {
+          const int64_t r = n - (c + 2) * kChunk;
+          const uint32_t bytes = (uint32_t)((r < kChunk ? r : kChunk) * 16);
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          mbar_expect_tx(&mbar[b], bytes);
+          bulk_load(buf, src + (c + 2) * kChunk, bytes, &mbar[b]);
         }
       }
+      (void)col_on;
     }
     __syncthreads();
     // ---- S3: box scan, in place ----
-    const int tpc = kThreads / ctot;  // threads per column
-    const int scol = tid % ctot, seg = tid / ctot;
+    constexpr int TPC = kThreads / CTOT;  // threads per column
+    const int scol = tid % CTOT, seg = tid / CTOT;
     float bnum = 0.f, bden = 1.f;
     int bm = prm.min_width, bj = 0;
     const bool scol_on = scol < ti.ncols;
     if (scol_on) {
       double f; int32_t nbk;
       freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, f, nbk);
-      const int per = (nbk + tpc - 1) / tpc;
+      const int per = (nbk + TPC - 1) / TPC;
       const int ja = seg * per;
       const int jb = min(nbk, ja + per);
       const uint32_t* hc = hist + scol;
@@ -209,8 +285,8 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
         for (int l = 0; l < MW - 1; ++l) {
           int e = ja + l;
           if (e >= nbk) e -= nbk;
-          ww[l] = (float)hc[e * stride] * inv_w;
-          ss[l] = (float)(int32_t)hc[e * stride + ctot];
+          ww[l] = (float)hc[e * STRIDE] * inv_w;
+          ss[l] = (float)(int32_t)hc[e * STRIDE + CTOT];
         }
         ww[MW - 1] = 0.f; ss[MW - 1] = 0.f;
         for (int j0 = ja; j0 < jb; j0 += MW) {
@@ -220,9 +296,14 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
             if (j < jb) {
               int e = j + MW - 1;
               if (e >= nbk) e -= nbk;
-              ww[(jj + MW - 1) % MW] = (float)hc[e * stride] * inv_w;
-              ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * stride + ctot];
+              ww[(jj + MW - 1) % MW] = (float)hc[e * STRIDE] * inv_w;
+              ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * STRIDE + CTOT];
               float r = ww[jj % MW], sm = ss[jj % MW];
+              if (wmask & 2u) {  // width 1 (not on the paper's ladder; kept for completeness)
+                const float d = fmaf(-r, r, r), num = sm * sm;
+                const float lhs = num * bden, rhs = bnum * d;
+                if (d > 0.f && (lhs > rhs || (lhs == rhs && 1 < bm))) { bnum = num; bden = d; bm = 1; bj = j; }
+              }
 #pragma unroll
               for (int m = 2; m <= MW; ++m) {
                 r += ww[(jj + m - 1) % MW];
@@ -234,12 +315,6 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
                   if (d > 0.f && (lhs > rhs || (lhs == rhs && m < bm))) { bnum = num; bden = d; bm = m; bj = j; }
                 }
               }
-              if (wmask & 2u) {  // width 1 (not on the paper's ladder; kept for completeness)
-                const float r1 = ww[jj % MW], s1 = ss[jj % MW];
-                const float d = fmaf(-r1, r1, r1), num = s1 * s1;
-                const float lhs = num * bden, rhs = bnum * d;
-                if (d > 0.f && (lhs > rhs || (lhs == rhs && 1 < bm))) { bnum = num; bden = d; bm = 1; bj = j; }
-              }
             }
           }
         }
@@ -250,11 +325,13 @@ __global__ void __launch_bounds__(kThreads) foldscan_kernel(
       float* cnum = reinterpret_cast<float*>(hist);
       float* cden = cnum + kThreads;
       uint32_t* cidx = hist + 2 * kThreads;
-      cnum[tid] = bnum; cden[tid] = bden; cidx[tid] = ((uint32_t)bm << 24) | (uint32_t)bj;
-      __syncthreads();
+      if (TPC > 1) {
+        cnum[tid] = bnum; cden[tid] = bden; cidx[tid] = ((uint32_t)bm << 24) | (uint32_t)bj;
+        __syncthreads();
+      }
       if (seg == 0 && scol_on) {
-        for (int g2 = 1; g2 < tpc; ++g2) {
-          const int o = g2 * ctot + scol;
+        for (int g2 = 1; g2 < TPC; ++g2) {
+          const int o = g2 * CTOT + scol;
           const float num = cnum[o], d = cden[o];
           const uint32_t idx = cidx[o];
           const int m = (int)(idx >> 24);
