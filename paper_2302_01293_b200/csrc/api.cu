@@ -141,7 +141,7 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
                 cudaSuccess &&                                                                                       \
             cudaFuncSetAttribute(foldscan_kernel<16, CT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
                 cudaSuccess
-  QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
+  QLP_ATTR(128); QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
   if (!attr_ok ||
       cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
@@ -308,7 +308,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   if (ctx->timing) CUDA_TRY(cudaEventRecord(ctx->ev0[slot], st));
   for (int c = 0; c < kNumClasses; ++c) {
     const size_t smem = (size_t)class_smem_bytes(c);
-    const int per_sm = (c == 0) ? 3 : (c == 1 ? 2 : 1);
+    const int per_sm = class_ctas_per_sm(c);
     const unsigned nblk = (unsigned)(ctx->n_sm * per_sm);
     const int64_t* off_c = off + (int64_t)c * (n_stars + 1);
     const bool wide = ctx->prm.max_width > 11;
@@ -318,6 +318,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
                                                          counters + c, sr, best)
 #define QLP_LAUNCH_MW(CT_) do { if (wide) QLP_LAUNCH(16, CT_); else QLP_LAUNCH(11, CT_); } while (0)
     switch (class_cols(c)) {
+      case 128: QLP_LAUNCH_MW(128); break;
       case 64: QLP_LAUNCH_MW(64); break;
       case 32: QLP_LAUNCH_MW(32); break;
       case 16: QLP_LAUNCH_MW(16); break;

@@ -18,7 +18,7 @@ namespace qlp {
 #define QLP_TWO52 4503599627370496.0
 
 constexpr int kMaxWidth = 16;     // largest supported box width in fine bins (ladder default: 11)
-constexpr int kThreads = 256;     // threads per CTA of the fold/scan kernel
+constexpr int kThreads = 512;     // threads per CTA of the fold/scan kernel
 constexpr int kWarps = kThreads / 32;
 constexpr int kNumClasses = 9;    // tile classes, see foldscan.cu
 constexpr int kMaxTopK = 8;
@@ -108,15 +108,16 @@ __device__ __forceinline__ int32_t bin_of(double f, double tau, double dnb, doub
 }
 
 // Tile classes of the fold/scan kernel: columns per CTA and the largest nb the class holds.
+// shared memory = cols * nbcap * 8 bytes of histograms + kStageBytes of point staging; class 0 fits
+// two CTAs per SM, the others one.
 __host__ __device__ __forceinline__ int class_cols(int c) {
-  return c <= 2 ? 64 : (32 >> (c - 3));
+  return c <= 1 ? 128 : (64 >> (c - 2));
 }
 __host__ __device__ __forceinline__ int class_nbcap(int c) {
-  // shared memory = cols * nbcap * 8 bytes of histograms + kStageBytes of point staging;
-  // class 0 fits 3 CTAs per SM, class 1 two, the others one.
-  const int caps[kNumClasses] = {116, 192, 420, 840, 1680, 3360, 6720, 13440, 24576};
+  const int caps[kNumClasses] = {94, 208, 420, 840, 1680, 3360, 6720, 13440, 24576};
   return caps[c];
 }
+__host__ __device__ __forceinline__ int class_ctas_per_sm(int c) { return c == 0 ? 2 : 1; }
 constexpr int kChunk = 512;                                   // points per staged chunk
 constexpr int kStageBytes = 2 * kChunk * 16 + 16;             // two buffers + two mbarriers
 __host__ __device__ __forceinline__ int class_smem_bytes(int c) {

@@ -126,30 +126,36 @@ struct TileInfo {
   int32_t valid;
 };
 
+
 // ---- the fused kernel ---------------------------------------------------------------------------
 // MW = widest box (window registers), CTOT = columns per CTA of this class (compile time so that the
 // two atomics of one evaluation differ by an immediate offset and the row stride is a shift).
+// Fold phase: every warp is a slice of the point stream.  With CTOT >= 32 a lane owns R = CTOT/32
+// columns (lane, lane+32, ...), so one broadcast LDS.128 of a point feeds R evaluations: the load
+// costs two shared-memory wavefronts, the two atomics of an evaluation one each, and the
+// shared-memory pipe (one wavefront per clock per SM) is what binds.
+// With CTOT < 32 the spare lanes take 32/CTOT consecutive points.
 template <int MW, int CTOT>
-__global__ void __launch_bounds__(kThreads, (CTOT == 64 ? 3 : 1)) foldscan_kernel(
+__global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kernel(
     Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const int64_t* __restrict__ tile_off, const int64_t* __restrict__ kb,
     unsigned long long* __restrict__ counter, float* __restrict__ sr, uint32_t* __restrict__ best) {
   extern __shared__ __align__(16) unsigned char smem[];
-  Point* pbuf = reinterpret_cast<Point*>(smem);                       // [2][kChunk]
+  Point* pbuf = reinterpret_cast<Point*>(smem);                          // [2][kChunk]
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem + 2 * kChunk * 16);  // [2]
-  uint32_t* hist = reinterpret_cast<uint32_t*>(smem + kStageBytes);   // [nb_tile][2 * CTOT]
+  uint32_t* hist = reinterpret_cast<uint32_t*>(smem + kStageBytes);      // [nb_tile][2 * CTOT]
   __shared__ TileInfo ti;
   constexpr int STRIDE = 2 * CTOT;              // words per histogram row: [W x CTOT][S x CTOT]
-  constexpr int CW = CTOT < 32 ? CTOT : 32;     // columns per warp
+  constexpr int CW = CTOT < 32 ? CTOT : 32;     // distinct columns across the lanes of a warp
+  constexpr int R = CTOT / CW;                  // columns per lane
   constexpr int HPW = 32 / CW;                  // points per warp iteration
-  constexpr int GROUPS = CTOT / CW;             // column groups (2 for 64 columns, else 1)
-  constexpr int NSLICES = kWarps / GROUPS;
-  constexpr int STEP = NSLICES * HPW;           // points consumed per iteration by one column group
+  constexpr int STEP = kWarps * HPW;            // points consumed per iteration by the CTA
   constexpr int ITERS = kChunk / STEP;
+  constexpr int U = ITERS < 4 ? ITERS : 4;      // points in flight per lane
+  static_assert(ITERS >= 1 && ITERS % U == 0, "chunk must be a multiple of the CTA's point step");
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int grp = warp % GROUPS, slice = warp / GROUPS;
-  const int col = grp * CW + (lane % CW);       // this lane's column in the fold phase
+  const int col0 = lane % CW;                   // first column of this lane in the fold phase
   const int hsub = lane / CW;
   const double dno = (double)prm.noverlap;
   const int64_t n_tiles = tile_off[n_stars];
@@ -218,16 +224,22 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 64 ? 3 : 1)) foldscan_kerne
     }
     // ---- S2: fold ----
     {
-      double f = 0.0; int32_t nbk = 1;
-      const bool col_on = col < ti.ncols;
-      if (col_on) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f, nbk);
-      const double dnb = (double)nbk, K = (dnb + 1.0) * QLP_TWO52;
+      // A column beyond the tile's last frequency folds with f = 0, nb = 1 into row 0 of its own
+      // (never scanned) column: cheaper than predicating every atomic.
+      double f[R], dnb[R], K[R];
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const int col = col0 + 32 * r;
+        f[r] = 0.0;
+        int32_t nbk = 1;
+        if (col < ti.ncols) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
+        dnb[r] = (double)nbk;
+        K[r] = (dnb[r] + 1.0) * QLP_TWO52;
+      }
       const int64_t n = ti.n_pts;
       const Point* src = pts + ti.pt_begin;
       const int64_t n_chunks = (n + kChunk - 1) / kChunk;
-      // a column that is switched off folds into its own (unused) cells with weight from the points;
-      // cheaper than predicating every atomic: its histogram is never scanned.
-      uint32_t* hcol = hist + col;
+      uint32_t* hcol = hist + col0;
       __syncthreads();  // histograms zeroed
       for (int64_t c = 0; c < n_chunks; ++c) {
         const int b = (int)(c & 1);
@@ -242,26 +254,33 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 64 ? 3 : 1)) foldscan_kerne
           }
           __syncthreads();
         }
-        const int4* p4 = reinterpret_cast<const int4*>(buf) + slice * HPW + hsub;
-#pragma unroll 8
-        for (int it = 0; it < ITERS; ++it) {
-          const int4 v = p4[it * STEP];
-          const double tau = __hiloint2double(v.y, v.x);
-          const int32_t bb = bin_of(f, tau, dnb, K);
-          uint32_t* cell = hcol + bb * STRIDE;
-          atomicAdd(cell, (uint32_t)v.z);
-          atomicAdd(cell + CTOT, (uint32_t)v.w);
+        const int4* p4 = reinterpret_cast<const int4*>(buf) + warp * HPW + hsub;
+#pragma unroll 1
+        for (int it = 0; it < ITERS; it += U) {
+          int4 v[U];
+#pragma unroll
+          for (int u = 0; u < U; ++u) v[u] = p4[(it + u) * STEP];
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const double tau = __hiloint2double(v[u].y, v[u].x);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+              const int32_t bb = bin_of(f[r], tau, dnb[r], K[r]);
+              uint32_t* cell = hcol + bb * STRIDE + 32 * r;
+              atomicAdd(cell, (uint32_t)v[u].z);
+              atomicAdd(cell + CTOT, (uint32_t)v[u].w);
+            }
+          }
         }
         __syncthreads();  // everyone is done with this buffer
         if (tid == 0 && c + 2 < n_chunks) {
-          const int64_t r = n - (c + 2) * kChunk;
-          const uint32_t bytes = (uint32_t)((r < kChunk ? r : kChunk) * 16);
+          const int64_t rr = n - (c + 2) * kChunk;
+          const uint32_t bytes = (uint32_t)((rr < kChunk ? rr : kChunk) * 16);
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           mbar_expect_tx(&mbar[b], bytes);
           bulk_load(buf, src + (c + 2) * kChunk, bytes, &mbar[b]);
         }
       }
-      (void)col_on;
     }
     __syncthreads();
     // ---- S3: box scan, in place ----
@@ -271,8 +290,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 64 ? 3 : 1)) foldscan_kerne
     int bm = prm.min_width, bj = 0;
     const bool scol_on = scol < ti.ncols;
     if (scol_on) {
-      double f; int32_t nbk;
-      freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, f, nbk);
+      double fk; int32_t nbk;
+      freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, fk, nbk);
       const int per = (nbk + TPC - 1) / TPC;
       const int ja = seg * per;
       const int jb = min(nbk, ja + per);
