@@ -146,6 +146,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem + 2 * kChunk * 16);  // [2]
   uint32_t* hist = reinterpret_cast<uint32_t*>(smem + kStageBytes);      // [nb_tile][2 * CTOT]
   __shared__ TileInfo ti;
+  __shared__ int64_t s_tile;
   constexpr int STRIDE = 2 * CTOT;              // words per histogram row: [W x CTOT][S x CTOT]
   constexpr int CW = CTOT < 32 ? CTOT : 32;     // distinct columns across the lanes of a warp
   constexpr int R = CTOT / CW;                  // columns per lane
@@ -169,16 +170,25 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
 
   for (;;) {
     __syncthreads();  // previous tile fully written before ti / hist are reused
+    if (tid == 0) s_tile = (int64_t)atomicAdd(counter, 1ull);
+    __syncthreads();
+    const int64_t tile = s_tile;
+    if (tile >= n_tiles) break;
+    // star of this tile = last s with tile_off[s] <= tile: a 512-way search, one global latency per level
+    int64_t lo = 0, len = n_stars + 1;
+    while (len > 1) {
+      const int64_t stride = (len + kThreads - 1) / kThreads;
+      const int64_t off = (int64_t)tid * stride;
+      const int hit = (off < len) && (tile_off[lo + off] <= tile);
+      const int c = __syncthreads_count(hit);
+      lo += (int64_t)(c - 1) * stride;
+      const int64_t rest = len - (int64_t)(c - 1) * stride;
+      len = stride < rest ? stride : rest;
+    }
     if (tid == 0) {
-      int64_t tile = (int64_t)atomicAdd(counter, 1ull);
       TileInfo x;
-      x.valid = tile < n_tiles;
-      if (x.valid) {
-        int64_t lo = 0, hi = n_stars - 1;  // last s with tile_off[s] <= tile
-        while (lo < hi) {
-          int64_t mid = lo + ((hi - lo + 1) >> 1);
-          if (tile_off[mid] <= tile) lo = mid; else hi = mid - 1;
-        }
+      x.valid = 1;
+      {
         const int64_t s = lo;
         const qlp_bls_star_grid g = grid[s];
         const StarPrep sp = prep[s];
@@ -214,7 +224,6 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       ti = x;
     }
     __syncthreads();
-    if (!ti.valid) break;
     const int nb_tile = ti.nb_tile;
     {  // zero the histograms of this tile
       const int words = nb_tile * STRIDE;  // multiple of 2; hist is 16-byte aligned
@@ -284,13 +293,18 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     }
     __syncthreads();
     // ---- S3: box scan, in place ----
+    // Each column is scanned by TPC threads, each over a contiguous range of start bins with the last
+    // MW bins held in registers (statically indexed ring).  Window sums are formed left to right,
+    // exactly as O4 states them.  The running maximum is kept as a value; a candidate is tested with
+    // one multiply and one compare (num > best * d) and the rare update takes a branch.
     constexpr int TPC = kThreads / CTOT;  // threads per column
     const int scol = tid % CTOT, seg = tid / CTOT;
-    float bnum = 0.f, bden = 1.f;
-    int bm = prm.min_width, bj = 0;
+    float bval = 0.f;
+    uint32_t bidx = (uint32_t)prm.min_width << 24;
     const bool scol_on = scol < ti.ncols;
+    int32_t nbk = 1;
     if (scol_on) {
-      double fk; int32_t nbk;
+      double fk;
       freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, fk, nbk);
       const int per = (nbk + TPC - 1) / TPC;
       const int ja = seg * per;
@@ -317,21 +331,17 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
               if (e >= nbk) e -= nbk;
               ww[(jj + MW - 1) % MW] = (float)hc[e * STRIDE] * inv_w;
               ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * STRIDE + CTOT];
-              float r = ww[jj % MW], sm = ss[jj % MW];
-              if (wmask & 2u) {  // width 1 (not on the paper's ladder; kept for completeness)
-                const float d = fmaf(-r, r, r), num = sm * sm;
-                const float lhs = num * bden, rhs = bnum * d;
-                if (d > 0.f && (lhs > rhs || (lhs == rhs && 1 < bm))) { bnum = num; bden = d; bm = 1; bj = j; }
-              }
+              float r = 0.f, sm = 0.f;
 #pragma unroll
-              for (int m = 2; m <= MW; ++m) {
+              for (int m = 1; m <= MW; ++m) {
                 r += ww[(jj + m - 1) % MW];
                 sm += ss[(jj + m - 1) % MW];
                 if ((wmask >> m) & 1u) {
                   const float d = fmaf(-r, r, r);  // r (1 - r)
                   const float num = sm * sm;
-                  const float lhs = num * bden, rhs = bnum * d;
-                  if (d > 0.f && (lhs > rhs || (lhs == rhs && m < bm))) { bnum = num; bden = d; bm = m; bj = j; }
+                  if (num > bval * d) {
+                    if (d > 0.f) { bval = __fdividef(num, d); bidx = ((uint32_t)m << 24) | (uint32_t)j; }
+                  }
                 }
               }
             }
@@ -339,29 +349,49 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         }
       }
     }
-    __syncthreads();  // all reads of hist done: reuse it as reduction scratch
-    {
-      float* cnum = reinterpret_cast<float*>(hist);
-      float* cden = cnum + kThreads;
-      uint32_t* cidx = hist + 2 * kThreads;
-      if (TPC > 1) {
-        cnum[tid] = bnum; cden[tid] = bden; cidx[tid] = ((uint32_t)bm << 24) | (uint32_t)bj;
-        __syncthreads();
+    // reduce over the TPC threads of a column (scratch = the idle staging buffers), earliest j wins ties
+    float* cval = reinterpret_cast<float*>(pbuf);
+    uint32_t* cidx = reinterpret_cast<uint32_t*>(pbuf) + kThreads;
+    if (TPC > 1) {
+      cval[tid] = bval; cidx[tid] = bidx;
+      __syncthreads();
+    }
+    if (seg == 0 && scol_on) {
+      for (int g2 = 1; g2 < TPC; ++g2) {
+        const float v = cval[g2 * CTOT + scol];
+        if (v > bval) { bval = v; bidx = cidx[g2 * CTOT + scol]; }
       }
-      if (seg == 0 && scol_on) {
-        for (int g2 = 1; g2 < TPC; ++g2) {
-          const int o = g2 * CTOT + scol;
-          const float num = cnum[o], d = cden[o];
-          const uint32_t idx = cidx[o];
-          const int m = (int)(idx >> 24);
-          const float lhs = num * bden, rhs = bnum * d;
-          // later segments hold larger j: they win only if strictly better, or equal with smaller m
-          if (lhs > rhs || (lhs == rhs && num > 0.f && m < bm)) { bnum = num; bden = d; bm = m; bj = (int)(idx & 0xffffffu); }
+      int bm = (int)(bidx >> 24), bj = (int)(bidx & 0xffffffu);
+      if (bval > 0.f) {
+        // Canonical representative of the winning box (O4 ties: smaller m, then smaller j).  Boxes
+        // that hold the same points have the same value; trim the empty bins off both ends, then
+        // take the narrowest ladder width that still covers the occupied span and, for it, the
+        // smallest start bin whose extra bins are all empty.
+        const uint32_t* hc = hist + scol;
+        auto empty = [&](int e) { e %= nbk; if (e < 0) e += nbk; return hc[e * STRIDE] == 0u; };
+        int a = bj, b = bj + bm - 1;
+        while (a < b && empty(a)) ++a;
+        while (b > a && empty(b)) --b;
+        const int mt = b - a + 1;
+        int el = 0, er = 0;  // empty bins next to the occupied span, as far as any box could reach
+        while (el < bm - mt && empty(a - 1 - el)) ++el;
+        while (er < bm - mt && empty(b + 1 + er)) ++er;
+        for (int m2 = mt; m2 <= bm; ++m2) {
+          if (!((prm.wmask >> m2) & 1u)) continue;
+          const int extra = m2 - mt;
+          int best_j = -1;
+          for (int x = 0; x <= extra; ++x) {  // x extra bins on the left, extra - x on the right
+            if (x > el || extra - x > er) continue;
+            int j = (a - x) % nbk;
+            if (j < 0) j += nbk;
+            if (best_j < 0 || j < best_j) best_j = j;
+          }
+          if (best_j >= 0) { bm = m2; bj = best_j; break; }
         }
-        const int64_t o = ti.out_base + ti.k0 + scol;
-        sr[o] = (bnum / bden) * ti.inv_s * ti.inv_s;
-        best[o] = ((uint32_t)bm << 24) | (uint32_t)bj;
       }
+      const int64_t o = ti.out_base + ti.k0 + scol;
+      sr[o] = (bval * ti.inv_s) * ti.inv_s;
+      best[o] = ((uint32_t)bm << 24) | (uint32_t)bj;
     }
   }
 }
