@@ -13,6 +13,8 @@
 
 using namespace qlp;
 
+static constexpr uint32_t kPaperMask = 0xFF8u;  // widths 3..11 (PAPER.md:19, :35 -> DESIGN.md O1.9)
+
 struct DevBuf {
   void* p = nullptr;
   size_t cap = 0;
@@ -137,9 +139,9 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
   bool attr_ok = true;
 #define QLP_ATTR(CT_)                                                                                                \
   attr_ok = attr_ok &&                                                                                               \
-            cudaFuncSetAttribute(foldscan_kernel<11, CT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
+            cudaFuncSetAttribute(foldscan_kernel<11, CT_, kPaperMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
                 cudaSuccess &&                                                                                       \
-            cudaFuncSetAttribute(foldscan_kernel<16, CT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
+            cudaFuncSetAttribute(foldscan_kernel<16, CT_, 0u>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
                 cudaSuccess
   QLP_ATTR(128); QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
   if (!attr_ok ||
@@ -311,12 +313,12 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
     const int per_sm = class_ctas_per_sm(c);
     const unsigned nblk = (unsigned)(ctx->n_sm * per_sm);
     const int64_t* off_c = off + (int64_t)c * (n_stars + 1);
-    const bool wide = ctx->prm.max_width > 11;
-#define QLP_LAUNCH(MW_, CT_)                                                                                          \
-  foldscan_kernel<MW_, CT_><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,    \
+    const bool generic = ctx->prm.wmask != kPaperMask;  // the paper's ladder {3..11} is compiled in
+#define QLP_LAUNCH(MW_, CT_, WM_)                                                                                          \
+  foldscan_kernel<MW_, CT_, WM_><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,    \
                                                          (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,    \
                                                          counters + c, sr, best)
-#define QLP_LAUNCH_MW(CT_) do { if (wide) QLP_LAUNCH(16, CT_); else QLP_LAUNCH(11, CT_); } while (0)
+#define QLP_LAUNCH_MW(CT_) do { if (generic) QLP_LAUNCH(16, CT_, 0u); else QLP_LAUNCH(11, CT_, kPaperMask); } while (0)
     switch (class_cols(c)) {
       case 128: QLP_LAUNCH_MW(128); break;
       case 64: QLP_LAUNCH_MW(64); break;

@@ -129,13 +129,14 @@ struct TileInfo {
 
 // ---- the fused kernel ---------------------------------------------------------------------------
 // MW = widest box (window registers), CTOT = columns per CTA of this class (compile time so that the
-// two atomics of one evaluation differ by an immediate offset and the row stride is a shift).
+// two atomics of one evaluation differ by an immediate offset and the row stride is a shift), WM = the
+// ladder as a compile-time bit mask (bit m set <=> width m is searched) or 0 = take it from prm.wmask.
 // Fold phase: every warp is a slice of the point stream.  With CTOT >= 32 a lane owns R = CTOT/32
 // columns (lane, lane+32, ...), so one broadcast LDS.128 of a point feeds R evaluations: the load
 // costs two shared-memory wavefronts, the two atomics of an evaluation one each, and the
 // shared-memory pipe (one wavefront per clock per SM) is what binds.
 // With CTOT < 32 the spare lanes take 32/CTOT consecutive points.
-template <int MW, int CTOT>
+template <int MW, int CTOT, uint32_t WM>
 __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kernel(
     Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
@@ -295,11 +296,11 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     // ---- S3: box scan, in place ----
     // Each column is scanned by TPC threads, each over a contiguous range of start bins with the last
     // MW bins held in registers (statically indexed ring).  Window sums are formed left to right,
-    // exactly as O4 states them.  The running maximum is kept as a value; a candidate is tested with
-    // one multiply and one compare (num > best * d) and the rare update takes a branch.
+    // exactly as O4 states them.  The running maximum is kept as a fraction (num, d) and updated with
+    // predicated moves: two multiplies and two compares per candidate, no division, no branch.
     constexpr int TPC = kThreads / CTOT;  // threads per column
     const int scol = tid % CTOT, seg = tid / CTOT;
-    float bval = 0.f;
+    float bnum = 0.f, bden = 1.f;  // running maximum as a fraction: no division in the scan
     uint32_t bidx = (uint32_t)prm.min_width << 24;
     const bool scol_on = scol < ti.ncols;
     int32_t nbk = 1;
@@ -311,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const int jb = min(nbk, ja + per);
       const uint32_t* hc = hist + scol;
       const float inv_w = ti.inv_w;
-      const uint32_t wmask = prm.wmask;
+      const uint32_t wmask = WM ? WM : prm.wmask;
       if (ja < jb) {
         float ww[MW], ss[MW];
 #pragma unroll
@@ -339,9 +340,12 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
                 if ((wmask >> m) & 1u) {
                   const float d = fmaf(-r, r, r);  // r (1 - r)
                   const float num = sm * sm;
-                  if (num > bval * d) {
-                    if (d > 0.f) { bval = __fdividef(num, d); bidx = ((uint32_t)m << 24) | (uint32_t)j; }
-                  }
+                  // branch-free running maximum of num/d by cross-multiplication (with 32 lanes a
+                  // warp-level "any lane improves" branch would be taken far too often)
+                  const bool up = (d > 0.f) && (num * bden > bnum * d);
+                  bnum = up ? num : bnum;
+                  bden = up ? d : bden;
+                  bidx = up ? (((uint32_t)m << 24) | (uint32_t)j) : bidx;
                 }
               }
             }
@@ -350,6 +354,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       }
     }
     // reduce over the TPC threads of a column (scratch = the idle staging buffers), earliest j wins ties
+    float bval = bnum / bden;
     float* cval = reinterpret_cast<float*>(pbuf);
     uint32_t* cidx = reinterpret_cast<uint32_t*>(pbuf) + kThreads;
     if (TPC > 1) {
@@ -377,7 +382,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         while (el < bm - mt && empty(a - 1 - el)) ++el;
         while (er < bm - mt && empty(b + 1 + er)) ++er;
         for (int m2 = mt; m2 <= bm; ++m2) {
-          if (!((prm.wmask >> m2) & 1u)) continue;
+          if (!(((WM ? WM : prm.wmask) >> m2) & 1u)) continue;
           const int extra = m2 - mt;
           int best_j = -1;
           for (int x = 0; x <= extra; ++x) {  // x extra bins on the left, extra - x on the right
