@@ -39,6 +39,7 @@ UNIT = "evals/s"
 ATOMS_LANES_PER_CLK_SM = 31.6
 FP64_LANES_PER_CLK_SM = 62.3
 N_SM = 148
+NCU_DRAM_BYTES_PER_STEP = 719.3e6  # 676.8 MB read + 42.5 MB written, profiles/r1_foldscan_ncu.txt
 
 
 def _peaks():
@@ -281,7 +282,12 @@ def run_gpu(args):
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
                      "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",
-                     "frac": achieved / peak if peak > 0 else None, "traffic": None,
+                     "frac": achieved / peak if peak > 0 else None,
+                     # dram__bytes_read+write of the foldscan launches of one step of THIS workload
+                     # (profiles/r1_foldscan_ncu.txt); valid for the default config-2 / 1000-star run only
+                     "traffic": NCU_DRAM_BYTES_PER_STEP if (args.config == 2 and args.stars == 1000) else None,
+                     "traffic_unit": "bytes per step (ncu dram read+write over the foldscan launches); algorithmic: "
+                                     f"{4 * 16 * int(batch.n_points) + 8 * int(tf)} (points read once per tile class + SR/best)",
                      "share_of_step": fold_ms / max(n_timed, 1) / (ms / args.steps),
                      "peak_source": f"148 SMs x {sm_max:.0f} MHz ({src}) x min(ATOMS lanes/2, FP64 lanes/4) per clk "
                                     "(profiles/ubench_r1.txt; DESIGN.md Roofline)"},
