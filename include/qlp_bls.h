@@ -184,8 +184,9 @@ int qlp_bls_debug_prep(qlp_bls_ctx* ctx, const int64_t* row_ptr, const double* t
                        const double* dy, const qlp_bls_star_grid* grid, int64_t star, double* tau,
                        float* w, float* wy, void* cuda_stream);
 
-/* Force one fold kernel for all frequencies: 0 = automatic (default), 1 = column kernel only
- * where it fits else wide, 2 = wide kernel everywhere.  Used by parity tests to cover both. */
+/* Force the tile class of the fold/scan kernel: 0 = automatic (default); p in 1..9 = no frequency may use a
+ * class below p - 1 (class c has 128, 128, 64, 32, 16, 8, 4, 2, 1 columns per CTA for c = 0..8), so that the
+ * narrow-column code paths, which real data reach only at very long baselines, are covered on small inputs. */
 int qlp_bls_debug_set_path(qlp_bls_ctx* ctx, int32_t path);
 
 #ifdef __cplusplus

@@ -223,7 +223,7 @@ extern "C" int qlp_bls_fold_elapsed_ms(qlp_bls_ctx* ctx, int32_t* n_calls, doubl
 }
 
 extern "C" int qlp_bls_debug_set_path(qlp_bls_ctx* ctx, int32_t path) {
-  if (!ctx || path < 0 || path > 3) return QLP_BLS_EINVAL;
+  if (!ctx || path < 0 || path > kNumClasses) return QLP_BLS_EINVAL;
   ctx->force_path = path;
   return QLP_BLS_OK;
 }

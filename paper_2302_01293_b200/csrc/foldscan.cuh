@@ -36,8 +36,7 @@ __global__ void tile_bounds_kernel(Params prm, int64_t n_stars, const qlp_bls_st
   for (int c = 0; c < kNumClasses; ++c) {
     int cap = class_nbcap(c);
     int64_t lo = 0, hi = nf;  // answer in [0, nf]
-    if (force_path == 2 && c < 3) lo = nf;       // test hook: push everything to the 32-column class
-    else if (force_path == 3 && c < 8) lo = nf;  // test hook: one column per CTA for everything
+    if (force_path > 0 && c < force_path - 1) lo = nf;  // test hook: nothing below class force_path - 1
     else {
       while (lo < hi) {
         int64_t mid = lo + ((hi - lo) >> 1);
@@ -149,6 +148,9 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
   __shared__ TileInfo ti;
   __shared__ int64_t s_tile;
   constexpr int STRIDE = 2 * CTOT;              // words per histogram row: [W x CTOT][S x CTOT]
+  constexpr int SB = (CTOT == 128) ? 10 : (CTOT == 64) ? 9 : (CTOT == 32) ? 8 : (CTOT == 16) ? 7 :
+                     (CTOT == 8) ? 6 : (CTOT == 4) ? 5 : (CTOT == 2) ? 4 : 3;  // log2(row bytes)
+  static_assert((1 << SB) == STRIDE * 4, "row bytes must be a power of two");
   constexpr int CW = CTOT < 32 ? CTOT : 32;     // distinct columns across the lanes of a warp
   constexpr int R = CTOT / CW;                  // columns per lane
   constexpr int HPW = 32 / CW;                  // points per warp iteration
@@ -244,12 +246,13 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         int32_t nbk = 1;
         if (col < ti.ncols) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
         dnb[r] = (double)nbk;
-        K[r] = (dnb[r] + 1.0) * QLP_TWO52;
+        K[r] = bin_offset_K2<SB>(dnb[r]);
       }
       const int64_t n = ti.n_pts;
       const Point* src = pts + ti.pt_begin;
       const int64_t n_chunks = (n + kChunk - 1) / kChunk;
-      uint32_t* hcol = hist + col0;
+      const uint32_t lane_off = (uint32_t)col0 * 4u;  // byte offset of this lane's first column in a row
+      unsigned char* hbytes = reinterpret_cast<unsigned char*>(hist);
       __syncthreads();  // histograms zeroed
       for (int64_t c = 0; c < n_chunks; ++c) {
         const int b = (int)(c & 1);
@@ -275,8 +278,9 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
             const double tau = __hiloint2double(v[u].y, v[u].x);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-              const int32_t bb = bin_of(f[r], tau, dnb[r], K[r]);
-              uint32_t* cell = hcol + bb * STRIDE + 32 * r;
+              // low word = bin * (row bytes) + fraction bits: one LOP3 clears them and adds the lane
+              const uint32_t off = (bin_offset_of<SB>(f[r], tau, dnb[r], K[r]) & ~((1u << SB) - 1u)) | lane_off;
+              uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + 32 * r;
               atomicAdd(cell, (uint32_t)v[u].z);
               atomicAdd(cell + CTOT, (uint32_t)v[u].w);
             }

@@ -188,7 +188,8 @@ def _check_best_valid(orc, cfg, b, go, s, ks, m_g, j_g, sr_o, tol):
         assert abs(v - sr_o[k]) <= 2 * tol, (s, k, v, sr_o[k], val)
 
 
-@pytest.mark.parametrize("name,path", [("c1", 0), ("c1", 2), ("c1", 3), ("c2", 0), ("c3", 0), ("c5", 0)])
+@pytest.mark.parametrize("name,path", [("c1", 0), ("c1", 2), ("c1", 3), ("c1", 4), ("c1", 5), ("c1", 6), ("c1", 7),
+                                       ("c1", 8), ("c1", 9), ("c2", 0), ("c3", 0), ("c5", 0), ("c5", 5)])
 def test_sr_parity_full(gpu, ctx, orc, cfg, batches, name, path):
     b = batches[name]
     if name == "c5":  # keep the oracle within seconds: the cheapest 12 of the 40 stars
@@ -251,6 +252,40 @@ def test_sr_parity_sampled_long_baseline(gpu, ctx, orc, cfg, batches):
             assert abs(g - v) <= SR_RTOL * peak, (s, int(k), int(nb[0]), g, v)
     # the sample must have reached the wide classes (nb > 880)
     assert go["nb_max"].max() > 880
+
+
+def test_sr_parity_sampled_config5_long_stars(gpu, ctx, orc, cfg):
+    """Config 5 (production-shaped): stars with many sectors reach nb ~ 2,700 (tile classes 4 and 5) and
+    ~2e5 points; the oracle is evaluated one frequency at a time on a sample."""
+    from paper_2302_01293_b200 import synth
+    b = synth.make_batch(5, star_ids=np.array([1, 19, 28]))
+    dev = gpu.upload(b)
+    grid, freq_ptr, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, tf)
+    sr, best, fp = sr.cpu().numpy(), best.cpu().numpy(), freq_ptr.cpu().numpy()
+    go = _oracle_grids(orc, cfg, b)
+    _assert_grid_equal(gpu.grid_to_numpy(grid), go)
+    M = orc.widths(cfg)
+    rng = np.random.default_rng(5)
+    assert go["nb_max"].max() > 1680
+    for s in range(b.n_stars):
+        nf = int(go[s]["n_freq"])
+        t, y, dy = b.star(s)
+        tau, w, wy = orc.prep(t, y, dy, float(go[s]["t_ref"]))
+        ks = np.unique(np.concatenate([[0, 1, nf - 1], (rng.random(40) ** 3 * nf).astype(np.int64),
+                                       rng.integers(0, nf, 20)]))
+        peak = float(sr[fp[s]:fp[s + 1]].max())
+        for k in ks:
+            f, nb = orc.freqs(cfg, go[s], int(k), int(k) + 1)
+            v, m, j, _, _ = orc.sr_one(tau, w, wy, float(f[0]), int(nb[0]), M)
+            g = float(sr[fp[s] + k])
+            assert abs(g - v) <= SR_RTOL * peak, (s, int(k), int(nb[0]), g, v)
+            bg = int(best[fp[s] + k])
+            if (bg >> 24, bg & 0xFFFFFF) != (m, j):  # a different box must be as good
+                bo = orc.bins(float(f[0]), int(nb[0]), tau)
+                sel = ((bo - (bg & 0xFFFFFF)) % int(nb[0])) < (bg >> 24)
+                r, sv = w[sel].sum(), wy[sel].sum()
+                assert abs(sv * sv / (r * (1 - r)) - v) <= 2 * SR_RTOL * peak
 
 
 def test_constant_and_degenerate_light_curves(gpu, ctx, orc, cfg):
