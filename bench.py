@@ -108,8 +108,7 @@ class ClockSampler:
 def make_workload(config: int, n_stars: int, rank: int):
     """Seeded synthetic batch; rank r takes star ids [r*n, (r+1)*n)."""
     from paper_2302_01293_b200 import synth
-    ids = np.arange(rank * n_stars, (rank + 1) * n_stars, dtype=np.int64)
-    return synth.make_batch(config, star_ids=ids)
+    return synth.make_batch(config, star_ids=shard_star_ids(n_stars, rank))
 
 
 def oracle_evals(orc, cfg, batch):
@@ -176,6 +175,23 @@ def run_reference(args):
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out))
+
+
+def shard_star_ids(n_stars_per_gpu: int, rank: int) -> np.ndarray:
+    """Stars are independent: rank r searches ids [r*n, (r+1)*n); no data-path collective."""
+    return np.arange(rank * n_stars_per_gpu, (rank + 1) * n_stars_per_gpu, dtype=np.int64)
+
+
+def aggregate_over_ranks(ms: float, e2e_ms: float, evals: int, stars: int, world: int, device: str):
+    """Whole-job figures: time = MAX over ranks, work = SUM over ranks (the only collective of the run)."""
+    if world <= 1:
+        return ms, e2e_ms, float(evals), float(stars)
+    import torch
+    import torch.distributed as dist
+    v = torch.tensor([ms, e2e_ms, float(evals), float(stars)], dtype=torch.float64, device=device)
+    mx = v.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+    sm = v.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+    return float(mx[0]), float(mx[1]), float(sm[2]), float(sm[3])
 
 
 def run_gpu(args):
@@ -250,13 +266,7 @@ def run_gpu(args):
     h2d = int(sum(a.nbytes for a in h))
     d2h = int(pk_host.nbytes)
 
-    tvals = torch.tensor([ms, e2e_s * 1e3, float(evals), float(S)], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        mx = tvals.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = tvals.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms, e2e_ms, evals_all, stars_all = float(mx[0]), float(mx[1]), float(sm[2]), float(sm[3])
-    else:
-        e2e_ms, evals_all, stars_all = e2e_s * 1e3, float(evals), float(S)
+    ms, e2e_ms, evals_all, stars_all = aggregate_over_ranks(ms, e2e_s * 1e3, evals, S, world, f"cuda:{local}")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
