@@ -57,6 +57,12 @@ def fold_peak_evals_per_s(sm_mhz: float) -> float:
     return N_SM * sm_mhz * 1e6 * per_clk_sm
 
 
+def fold_issue_bound_evals_per_s(sm_mhz: float) -> float:
+    """Tighter bound: an FP64 instruction costs its scheduler 2 issue cycles and nothing issues in its shadow
+    (profiles/ubench_r1.txt), so 32 evaluations cost >= 4*2 + 1 (address) + 2 (ATOMS) + 0.25 (LDS) cycles."""
+    return N_SM * sm_mhz * 1e6 * 4 * 32 / 11.25
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -293,6 +299,8 @@ def run_gpu(args):
         "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
                      "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",
                      "frac": achieved / peak if peak > 0 else None,
+                     "issue_bound": fold_issue_bound_evals_per_s(sm_max) / 1e9,
+                     "frac_of_issue_bound": achieved / fold_issue_bound_evals_per_s(sm_max),
                      # dram__bytes_read+write of the foldscan launches of one step of THIS workload
                      # (profiles/r1_foldscan_ncu.txt); valid for the default config-2 / 1000-star run only
                      "traffic": NCU_DRAM_BYTES_PER_STEP if (args.config == 2 and args.stars == 1000) else None,

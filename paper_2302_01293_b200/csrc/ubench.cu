@@ -70,6 +70,33 @@ __global__ void k_bin(int iters, long long* cyc, int* sink) {
   sink[blockIdx.x * blockDim.x + t] = acc;
 }
 
+// Issue cost next to the FP64 pipe: 4 DFMA per iteration plus NI independent 32-bit logic ops (LOP3).  If the
+// logic ops issued in the shadow of the half-rate DFMAs the time would not grow with NI; it does (additively),
+// i.e. an FP64 instruction occupies its scheduler for two issue cycles.
+template <int NI>
+__global__ void k_mix(int iters, long long* cyc, double* sink) {
+  const int t = threadIdx.x;
+  double a0 = 1.0 + t * 1e-3, a1 = 1.1, a2 = 1.2, a3 = 1.3;
+  const double m = 1.0000001, c = 1e-9;
+  unsigned i0 = t, i1 = 3, i2 = 5, i3 = 7, i4 = 11, i5 = 13, i6 = 17, i7 = 19;
+  const unsigned q = (blockIdx.x << 7) | 0x55u;
+  long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    if (NI >= 1) i0 = (i0 & q) ^ (unsigned)it;
+    if (NI >= 2) i1 = (i1 | q) ^ (unsigned)it;
+    if (NI >= 3) i2 = (i2 & q) ^ (unsigned)it;
+    if (NI >= 4) i3 = (i3 | q) ^ (unsigned)it;
+    if (NI >= 5) i4 = (i4 & q) ^ (unsigned)it;
+    if (NI >= 6) i5 = (i5 | q) ^ (unsigned)it;
+    if (NI >= 7) i6 = (i6 & q) ^ (unsigned)it;
+    if (NI >= 8) i7 = (i7 | q) ^ (unsigned)it;
+  }
+  long long t1 = clock64();
+  if (t == 0) cyc[blockIdx.x] = t1 - t0;
+  sink[blockIdx.x * blockDim.x + t] = a0 + a1 + a2 + a3 + (double)(i0 + i1 + i2 + i3 + i4 + i5 + i6 + i7);
+}
+
 template <typename F>
 static double run(F launch, int nblk, long long* cyc) {
   launch(); launch();
@@ -105,9 +132,14 @@ int main() {
     if (v > best_bin) best_bin = v;
   }
   (void)threads;
+  // cycles per warp iteration per scheduler (1024 threads = 8 warps per scheduler)
+  const double mix0 = run([&] { k_mix<0><<<nsm, 1024>>>(iters, cyc, (double*)sink); }, nsm, cyc) / iters / 8.0;
+  const double mix4 = run([&] { k_mix<4><<<nsm, 1024>>>(iters, cyc, (double*)sink); }, nsm, cyc) / iters / 8.0;
+  const double mix8 = run([&] { k_mix<8><<<nsm, 1024>>>(iters, cyc, (double*)sink); }, nsm, cyc) / iters / 8.0;
   int clk_khz = 0;
   cudaDeviceGetAttribute(&clk_khz, cudaDevAttrClockRate, 0);
   printf("{\"sms\": %d, \"sm_max_mhz\": %.0f, \"atoms_lanes_per_clk_sm\": %.2f, \"fp64_lanes_per_clk_sm\": %.2f, "
-         "\"bin_evals_per_clk_sm\": %.2f}\n", nsm, clk_khz / 1000.0, best_atoms, best_fp64, best_bin);
+         "\"bin_evals_per_clk_sm\": %.2f, \"issue_cycles_4dfma\": %.2f, \"issue_cycles_4dfma_4lop3\": %.2f, "
+         "\"issue_cycles_4dfma_8lop3\": %.2f}\n", nsm, clk_khz / 1000.0, best_atoms, best_fp64, best_bin, mix0, mix4, mix8);
   return cudaGetLastError() == cudaSuccess ? 0 : 2;
 }
