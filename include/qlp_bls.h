@@ -60,7 +60,10 @@ typedef struct {
   double qmax_fac;          /* 2.0                                                 */
   double a_over_rstar_min;  /* 2.0 (3.0 = the Sectors 59-60 variant)                */
   double sector_days;       /* 27.4                                                  */
-  uint32_t flags;           /* bit0: validate inputs on the device; other bits reserved (0)      */
+  uint32_t flags;           /* bit0: validate inputs on the device (t finite and strictly
+                               increasing in qlp_bls_grid; y, dy finite and dy > 0 in
+                               qlp_bls_spectrum, which then synchronises once); a violation makes
+                               the call return QLP_BLS_EVALIDATION.  Other bits reserved (0)      */
   uint32_t reserved_;       /* 0                                                                 */
 } qlp_bls_config;
 

@@ -228,6 +228,19 @@ extern "C" int qlp_bls_debug_set_path(qlp_bls_ctx* ctx, int32_t path) {
   return QLP_BLS_OK;
 }
 
+// flags bit0: count invalid inputs on the device; one synchronising read-back (totals_host[3])
+static int run_validation(qlp_bls_ctx* ctx, int which, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                          const double* y, const double* dy, cudaStream_t st) {
+  if (!(ctx->cfg.flags & 1u) || n_stars == 0) return 0;
+  unsigned long long* bad = (unsigned long long*)ctx->totals_dev.p + 3;
+  CUDA_TRY(cudaMemsetAsync(bad, 0, 8, st));
+  validate_kernel<<<(unsigned)n_stars, 256, 0, st>>>(which, n_stars, row_ptr, t, y, dy, bad);
+  QLP_TRY(launch_ok(ctx));
+  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 3, bad, 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return ctx->totals_host[3] != 0 ? QLP_BLS_EVALIDATION : 0;
+}
+
 // ---- S1 -----------------------------------------------------------------------------------------
 extern "C" int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                             const double* rho, const double* rstar, qlp_bls_star_grid* grid, int64_t* freq_ptr,
@@ -239,6 +252,7 @@ extern "C" int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* ro
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(ctx->device));
   QLP_TRY(ctx->star_bins.ensure((size_t)(n_stars + 1) * 8));
+  QLP_TRY(run_validation(ctx, 0, n_stars, row_ptr, t, nullptr, nullptr, st));
   if (n_stars > 0) {
     grid_kernel<<<(unsigned)n_stars, 256, 0, st>>>(ctx->prm, n_stars, row_ptr, t, rho, grid,
                                                   (unsigned long long*)ctx->star_bins.p);
@@ -292,6 +306,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   if (n_stars > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(ctx->device));
+  QLP_TRY(run_validation(ctx, 1, n_stars, row_ptr, t, y, dy, st));
   QLP_TRY(run_prep(ctx, n_stars, row_ptr, t, y, dy, grid, st));
   QLP_TRY(ctx->kb.ensure((size_t)n_stars * kNumClasses * 8));
   QLP_TRY(ctx->cnt.ensure((size_t)n_stars * kNumClasses * 8));

@@ -119,6 +119,30 @@ __global__ void __launch_bounds__(256) prep_kernel(Params prm, int64_t n_stars, 
   }
 }
 
+// Optional input validation (config flags bit0).  which = 0: t finite and strictly increasing within each star,
+// row_ptr non-decreasing; which = 1: y finite, dy finite and > 0.  Counts violations into *bad.
+__global__ void validate_kernel(int which, int64_t n_stars, const int64_t* __restrict__ row_ptr,
+                                const double* __restrict__ t, const double* __restrict__ y,
+                                const double* __restrict__ dy, unsigned long long* __restrict__ bad) {
+  const int64_t s = blockIdx.x;
+  if (s >= n_stars) return;
+  const int64_t a = row_ptr[s], n = row_ptr[s + 1] - a;
+  unsigned long long cnt = 0;
+  if (n < 0) cnt = 1;
+  for (int64_t i = threadIdx.x; i < n; i += blockDim.x) {
+    if (which == 0) {
+      const double ti = t[a + i];
+      if (!isfinite(ti)) ++cnt;
+      if (i + 1 < n && !(t[a + i + 1] > ti)) ++cnt;
+    } else {
+      const double d = dy[a + i];
+      if (!isfinite(y[a + i]) || !isfinite(d) || !(d > 0.0)) ++cnt;
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+  if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(bad, cnt);
+}
+
 // test-only: S0 outputs of one star as plain arrays
 __global__ void debug_prep_kernel(const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
                                   const StarPrep* __restrict__ prep, int64_t star, double* __restrict__ tau,

@@ -1,0 +1,131 @@
+"""Edge cases and full-size checks of the CUDA path (run with -m gpu).
+
+  * flags bit0 input validation (QLP_BLS_EVALIDATION);
+  * a star that would need more phase bins than QLP_BLS_MAX_NB is skipped with status 4, its neighbours untouched;
+  * the exact launch configuration bench.py times (BASELINE.json configs[1]: 1,000 stars) checked against the
+    oracle on sampled (star, frequency) outputs and on whole spectra of a few stars.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SR_RTOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2302_01293_b200 import build, bls
+    build.build()
+    return bls
+
+
+def test_validation_flag(gpu):
+    from paper_2302_01293_b200 import synth
+    t = synth.sector_times(0, 1800.0)
+    rng = np.random.default_rng(0)
+    good = (t, rng.standard_normal(t.size) * 1e-3, np.full(t.size, 1e-3))
+    ctx = gpu.QlpBls(flags=1)
+    try:
+        dev = gpu.upload(synth.from_arrays([good, good]))
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)  # valid inputs pass
+        t_bad = t.copy(); t_bad[100] = t_bad[99]                    # not strictly increasing
+        dev = gpu.upload(synth.from_arrays([good, (t_bad, good[1], good[2])]))
+        with pytest.raises(gpu.QlpBlsError, match="validation"):
+            ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        dy_bad = good[2].copy(); dy_bad[5] = 0.0                    # dy must be > 0
+        dev = gpu.upload(synth.from_arrays([good, (t, good[1], dy_bad)]))
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        with pytest.raises(gpu.QlpBlsError, match="validation"):
+            ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        y_bad = good[1].copy(); y_bad[7] = np.nan
+        dev = gpu.upload(synth.from_arrays([(t, y_bad, good[2])]))
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        with pytest.raises(gpu.QlpBlsError, match="validation"):
+            ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+    finally:
+        ctx.close()
+
+
+def test_star_above_bin_cap_is_skipped(gpu, orc, cfg):
+    """70 contiguous 30-min sectors and a very dense star: nb at the longest period exceeds QLP_BLS_MAX_NB."""
+    from paper_2302_01293_b200 import synth
+    t_long = np.concatenate([synth.sector_times(s, 1800.0) for s in range(70)])
+    rng = np.random.default_rng(1)
+    mk = lambda t: (t, rng.standard_normal(t.size) * 1e-3, np.full(t.size, 1e-3))
+    t_short = synth.sector_times(0, 1800.0)
+    b = synth.from_arrays([mk(t_short), mk(t_long), mk(t_short)], rho=np.array([1.0, 200.0, 1.0]))
+    ctx = gpu.QlpBls()
+    try:
+        dev = gpu.upload(b)
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        g = gpu.grid_to_numpy(grid)
+        go = orc.grid(cfg, t_long, 200.0)
+        assert go["nb_max"] > 24576                       # the oracle's descriptor says so too
+        assert g["status"].tolist() == [0, 4, 0] and g["n_freq"][1] == 0
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        snr, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best)
+        pk = gpu.peaks_to_numpy(peaks, ctx.top_k)
+        assert pk[1][0]["k"] == -1 and pk[0][0]["k"] >= 0 and pk[2][0]["k"] >= 0
+        # the neighbours are unaffected: identical inputs -> identical spectra
+        fpn = fp.cpu().numpy()
+        s0 = sr[fpn[0]:fpn[1]].cpu().numpy()
+        so, _, _ = orc.spectrum_star(cfg, orc.grid(cfg, t_short, 1.0), *b.star(0))
+        assert np.abs(s0 - so).max() <= SR_RTOL * so.max()
+    finally:
+        ctx.close()
+
+
+def test_bench_configuration_sampled(gpu, orc, cfg):
+    """BASELINE.json configs[1] at full size (1,000 stars), in the launch configuration bench.py times."""
+    from paper_2302_01293_b200 import synth
+    b = synth.make_batch(2, n_stars=1000)
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        dev = gpu.upload(b)
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        snr, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best)
+        g = gpu.grid_to_numpy(grid)
+        sr, fpn, snr = sr.cpu().numpy(), fp.cpu().numpy(), snr.cpu().numpy()
+        pk = gpu.peaks_to_numpy(peaks, ctx.top_k)
+        assert np.all(g["status"] == 0) and np.all(np.isfinite(sr)) and np.all(sr >= 0)
+        M = orc.widths(cfg)
+        rng = np.random.default_rng(2)
+        # (a) 60 sampled (star, frequency) outputs, one oracle evaluation each
+        for s in rng.integers(0, 1000, 20):
+            t, y, dy = b.star(int(s))
+            go = orc.grid(cfg, t, float(b.rho[s]))
+            assert go.tobytes() == g[s].tobytes()
+            tau, w, wy = orc.prep(t, y, dy, float(go["t_ref"]))
+            peak = float(sr[fpn[s]:fpn[s + 1]].max())
+            for k in rng.integers(0, int(go["n_freq"]), 3):
+                f, nb = orc.freqs(cfg, go, int(k), int(k) + 1)
+                v = orc.sr_one(tau, w, wy, float(f[0]), int(nb[0]), M)[0]
+                assert abs(float(sr[fpn[s] + k]) - v) <= SR_RTOL * peak
+        # (b) three whole stars: spectrum, S/N and top peak
+        for s in (0, 499, 999):
+            t, y, dy = b.star(s)
+            go = orc.grid(cfg, t, float(b.rho[s]))
+            so, mo, jo = orc.spectrum_star(cfg, go, t, y, dy)
+            assert np.abs(sr[fpn[s]:fpn[s + 1]] - so).max() <= SR_RTOL * so.max()
+            sn_o, _, _ = orc.snr(orc.freqs(cfg, go)[0], so)
+            scale = np.abs(sn_o).max()
+            assert np.abs(snr[fpn[s]:fpn[s + 1]] - sn_o).max() <= 5e-4 * scale + 1e-3
+            top2 = np.sort(sn_o)[-2:]
+            if top2[1] - top2[0] > 1e-3 * scale:
+                assert pk[s][0]["k"] == int(np.argmax(sn_o))
+        # (c) properties that hold at any size: injected transits are recovered at the right period
+        inj = np.nonzero(b.truth["period"] > 0)[0]
+        deep = [s for s in inj if b.truth["depth"][s] > 20 * np.median(b.star(int(s))[2]) / np.sqrt(50)]
+        hits = 0
+        for s in deep:
+            ratio = pk[s][0]["period"] / b.truth["period"][s]
+            hits += any(abs(ratio - h) < 0.02 * h for h in (0.5, 1.0, 2.0, 1 / 3, 3.0))
+        assert len(deep) > 20 and hits >= 0.8 * len(deep), (hits, len(deep))
+    finally:
+        ctx.close()
