@@ -257,6 +257,7 @@ def run_gpu(args):
     clocks = sampler.stop() if rank == 0 else None
     ms = e0.elapsed_time(e1)
     n_timed, fold_ms = ctx.fold_elapsed_ms()
+    ph = ctx.fold_phase_clocks()
     ctx.fold_timing(False)
 
     # end to end through the host-buffer API: pinned host inputs, H2D and D2H inside the timed region
@@ -299,6 +300,10 @@ def run_gpu(args):
         "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
                      "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",
                      "frac": achieved / peak if peak > 0 else None,
+                     # thread-0 SM clocks per phase of the fused kernel, summed over all tiles of the timed steps
+                     "phase_share": {"setup_zero": ph[0] / max(sum(ph), 1), "fold_S2": ph[1] / max(sum(ph), 1),
+                                     "scan_S3": ph[2] / max(sum(ph), 1)},
+                     "fold_only_achieved": achieved / 1e9 / max(ph[1] / max(sum(ph), 1), 1e-9),
                      "issue_bound": fold_issue_bound_evals_per_s(sm_max) / 1e9,
                      "frac_of_issue_bound": achieved / fold_issue_bound_evals_per_s(sm_max),
                      # dram__bytes_read+write of the foldscan launches of one step of THIS workload

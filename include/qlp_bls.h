@@ -166,6 +166,11 @@ int qlp_bls_fold_timing(qlp_bls_ctx* ctx, int32_t enable);
  * time of their fold/scan launches. */
 int qlp_bls_fold_elapsed_ms(qlp_bls_ctx* ctx, int32_t* n_calls /*host*/, double* total_ms /*host*/);
 
+/* While fold timing is on, the fold/scan kernel also adds up thread 0's SM clocks per phase over all tiles:
+ * clocks[0] = tile set-up + zeroing, clocks[1] = fold (S2), clocks[2] = box scan + reduction + output (S3).
+ * Their ratios split the fused kernel's time between S2 and S3.  Synchronises the device.  clocks host [3]. */
+int qlp_bls_fold_phase_clocks(qlp_bls_ctx* ctx, uint64_t* clocks /*host*/);
+
 /* The duration ladder in fine bins (O1.9): writes up to cap widths to m (host),
  * returns their number. */
 int qlp_bls_widths(const qlp_bls_ctx* ctx, int32_t* m /*host*/, int32_t cap);

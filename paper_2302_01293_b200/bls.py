@@ -36,7 +36,7 @@ PEAK_DTYPE = np.dtype([("k", "i8"), ("freq", "f8"), ("period", "f8"), ("t0", "f8
 
 EXPORTS = ["qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
-           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
+           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
 
 _lib = None
@@ -70,6 +70,7 @@ def load_library():
         L.qlp_bls_debug_set_path.argtypes = [vp, i32]
         L.qlp_bls_fold_timing.argtypes = [vp, i32]
         L.qlp_bls_fold_elapsed_ms.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_double)]
+        L.qlp_bls_fold_phase_clocks.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -143,6 +144,12 @@ class QlpBls:
         n, ms = C.c_int32(), C.c_double()
         _check(self.lib.qlp_bls_fold_elapsed_ms(self._h, C.byref(n), C.byref(ms)), "qlp_bls_fold_elapsed_ms")
         return int(n.value), float(ms.value)
+
+    def fold_phase_clocks(self):
+        """-> (set-up, fold, scan) SM clocks of thread 0 summed over all tiles since fold_timing(True)."""
+        a = np.zeros(3, dtype=np.uint64)
+        _check(self.lib.qlp_bls_fold_phase_clocks(self._h, a.ctypes.data_as(C.c_void_p)), "qlp_bls_fold_phase_clocks")
+        return [int(x) for x in a]
 
     def debug_set_path(self, path: int):
         _check(self.lib.qlp_bls_debug_set_path(self._h, path), "qlp_bls_debug_set_path")

@@ -151,7 +151,7 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
   if (cudaMallocHost((void**)&ctx->totals_host, 4 * sizeof(int64_t)) != cudaSuccess) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ENOMEM;
   }
-  if (ctx->totals_dev.ensure(4 * sizeof(int64_t)) != 0) { cudaFreeHost(ctx->totals_host); delete ctx; return QLP_BLS_ENOMEM; }
+  if (ctx->totals_dev.ensure(8 * sizeof(int64_t)) != 0) { cudaFreeHost(ctx->totals_host); delete ctx; return QLP_BLS_ENOMEM; }
   *out = ctx;
   return QLP_BLS_OK;
 }
@@ -203,6 +203,15 @@ extern "C" int qlp_bls_fold_timing(qlp_bls_ctx* ctx, int32_t enable) {
   }
   ctx->timing = enable != 0;
   ctx->ev_calls = 0;
+  CUDA_TRY(cudaMemset((unsigned long long*)ctx->totals_dev.p + 4, 0, 3 * 8));
+  return QLP_BLS_OK;
+}
+
+extern "C" int qlp_bls_fold_phase_clocks(qlp_bls_ctx* ctx, uint64_t* clocks) {
+  if (!ctx || !clocks) return QLP_BLS_EINVAL;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  CUDA_TRY(cudaMemcpy(clocks, (unsigned long long*)ctx->totals_dev.p + 4, 3 * 8, cudaMemcpyDeviceToHost));
   return QLP_BLS_OK;
 }
 
@@ -317,6 +326,8 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   int64_t* off = (int64_t*)ctx->off.p;
   unsigned long long* counters = (unsigned long long*)ctx->counters.p;
   CUDA_TRY(cudaMemsetAsync(counters, 0, kNumClasses * 8, st));
+  // per-phase clock counters of the fold/scan kernel (only while fold timing is on)
+  unsigned long long* phase = ctx->timing ? (unsigned long long*)ctx->totals_dev.p + 4 : nullptr;
   tile_bounds_kernel<<<(unsigned)((n_stars + 127) / 128), 128, 0, st>>>(ctx->prm, n_stars, grid, ctx->force_path, kb, cnt);
   QLP_TRY(launch_ok(ctx));
   tile_scan_kernel<<<kNumClasses, 1024, 0, st>>>(n_stars, cnt, off);
@@ -332,7 +343,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
 #define QLP_LAUNCH(MW_, CT_, WM_)                                                                                          \
   foldscan_kernel<MW_, CT_, WM_><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,    \
                                                          (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,    \
-                                                         counters + c, sr, best)
+                                                         counters + c, sr, best, phase)
 #define QLP_LAUNCH_MW(CT_) do { if (generic) QLP_LAUNCH(16, CT_, 0u); else QLP_LAUNCH(11, CT_, kPaperMask); } while (0)
     switch (class_cols(c)) {
       case 128: QLP_LAUNCH_MW(128); break;

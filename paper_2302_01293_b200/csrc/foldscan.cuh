@@ -140,7 +140,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const int64_t* __restrict__ tile_off, const int64_t* __restrict__ kb,
-    unsigned long long* __restrict__ counter, float* __restrict__ sr, uint32_t* __restrict__ best) {
+    unsigned long long* __restrict__ counter, float* __restrict__ sr, uint32_t* __restrict__ best,
+    unsigned long long* __restrict__ phase /* NULL, or 3 counters: set-up, fold, scan clocks of thread 0 */) {
   extern __shared__ __align__(16) unsigned char smem[];
   Point* pbuf = reinterpret_cast<Point*>(smem);                          // [2][kChunk]
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem + 2 * kChunk * 16);  // [2]
@@ -173,6 +174,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
 
   for (;;) {
     __syncthreads();  // previous tile fully written before ti / hist are reused
+    const long long clk0 = phase ? clock64() : 0;
     if (tid == 0) s_tile = (int64_t)atomicAdd(counter, 1ull);
     __syncthreads();
     const int64_t tile = s_tile;
@@ -234,6 +236,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       for (int i = tid; i < (words >> 2); i += kThreads) h4[i] = make_uint4(0u, 0u, 0u, 0u);
       if (tid < (words & 3)) hist[(words & ~3) + tid] = 0u;
     }
+    long long clk1s = 0;
     // ---- S2: fold ----
     {
       // A column beyond the tile's last frequency folds with f = 0, nb = 1 into row 0 of its own
@@ -254,6 +257,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const uint32_t lane_off = (uint32_t)col0 * 4u;  // byte offset of this lane's first column in a row
       unsigned char* hbytes = reinterpret_cast<unsigned char*>(hist);
       __syncthreads();  // histograms zeroed
+      clk1s = phase ? clock64() : 0;
       for (int64_t c = 0; c < n_chunks; ++c) {
         const int b = (int)(c & 1);
         Point* buf = pbuf + b * kChunk;
@@ -297,6 +301,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       }
     }
     __syncthreads();
+    const long long clk2 = phase ? clock64() : 0;
     // ---- S3: box scan, in place ----
     // Each column is scanned by TPC threads, each over a contiguous range of start bins with the last
     // MW bins held in registers (statically indexed ring).  Window sums are formed left to right,
@@ -401,6 +406,12 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const int64_t o = ti.out_base + ti.k0 + scol;
       sr[o] = (bval * ti.inv_s) * ti.inv_s;
       best[o] = ((uint32_t)bm << 24) | (uint32_t)bj;
+    }
+    if (phase && tid == 0) {  // thread 0's clocks: tile set-up + zeroing, fold, scan + reduction + output
+      const long long clk3 = clock64();
+      atomicAdd(&phase[0], (unsigned long long)(clk1s - clk0));
+      atomicAdd(&phase[1], (unsigned long long)(clk2 - clk1s));
+      atomicAdd(&phase[2], (unsigned long long)(clk3 - clk2));
     }
   }
 }
