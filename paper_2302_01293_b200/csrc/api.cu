@@ -44,7 +44,10 @@ struct qlp_bls_ctx {
   // workspace
   DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev;
   // host-API staging
-  DevBuf h_row, h_t, h_y, h_dy, h_rho, h_grid, h_fptr, h_sr, h_best, h_peaks;
+  DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks;
+  cudaStream_t copy_stream = nullptr;  // H2D of the next sub-batch overlaps the search of the current one
+  cudaEvent_t h2d_done[2], set_free[2];
+  bool copy_ready = false;
   int64_t* totals_host = nullptr;  // pinned, 4 x int64
   // cache of the last grid call: lets spectrum/snr size the point workspace without a sync
   const int64_t* last_row_ptr = nullptr;
@@ -160,10 +163,15 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   if (!ctx) return QLP_BLS_OK;
   cudaSetDevice(ctx->device);
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
-                    &ctx->totals_dev, &ctx->h_row, &ctx->h_t, &ctx->h_y, &ctx->h_dy, &ctx->h_rho, &ctx->h_grid,
+                    &ctx->totals_dev, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
+                    &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks};
   for (DevBuf* b : bufs) b->release();
   if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
+  if (ctx->copy_ready) {
+    cudaStreamDestroy(ctx->copy_stream);
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(ctx->h2d_done[i]); cudaEventDestroy(ctx->set_free[i]); }
+  }
   if (ctx->ev_ready)
     for (int i = 0; i < qlp_bls_ctx::kRing; ++i) { cudaEventDestroy(ctx->ev0[i]); cudaEventDestroy(ctx->ev1[i]); }
   delete ctx;
@@ -379,9 +387,12 @@ extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row
 }
 
 // ---- whole path from host buffers -------------------------------------------------------------------
-// Stars are processed in chunks bounded by a point budget so that the device copies stay small next
-// to 180 GB of HBM: per chunk H2D (row_ptr rebased, t, y, dy, rho) -> grid -> spectrum -> snr -> D2H
-// of the peak table only.
+// Stars are processed in sub-batches: per sub-batch H2D (row_ptr rebased, t, y, dy, rho) -> grid -> spectrum ->
+// snr -> D2H of the peak table only.  The H2D of sub-batch i+1 runs on the context's copy stream into the
+// second set of staging buffers while sub-batch i is searched, so with pinned host memory only the first
+// sub-batch's copy is exposed.  Sub-batch size: enough points to keep the persistent fold kernels busy, small
+// enough for several sub-batches per call, and never more than a point budget that keeps the device copies
+// small next to 180 GB of HBM.
 extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                    const double* y, const double* dy, const double* rho, const double* rstar,
                                    qlp_bls_peak* peaks, qlp_bls_star_grid* grid_out, int64_t* total_freq,
@@ -391,67 +402,125 @@ extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int6
   if (n_stars > 0 && (!t || !y || !dy || !rho)) return QLP_BLS_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(ctx->device));
+  if (total_freq) *total_freq = 0;
+  if (n_stars == 0) return QLP_BLS_OK;
+  if (!ctx->copy_ready) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CUDA_TRY(cudaEventCreateWithFlags(&ctx->h2d_done[i], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&ctx->set_free[i], cudaEventDisableTiming));
+    }
+    ctx->copy_ready = true;
+  }
   const int K = ctx->prm.top_k;
-  const int64_t kPointBudget = 256ll << 20;  // points per chunk (4 GiB of point records)
+  const int64_t n_points = row_ptr[n_stars] - row_ptr[0];
+  if (n_points < 0) return QLP_BLS_EINVAL;
+  // a small first sub-batch (its copy is the only exposed one), then about three large ones (each sub-batch
+  // costs a synchronising grid call and the tail of the persistent fold kernels)
+  auto clamp_budget = [](int64_t b) {
+    if (b < (1ll << 20)) b = 1ll << 20;          // at least 1 M points (24 MB of input)
+    if (b > (256ll << 20)) b = 256ll << 20;      // at most 256 M points (4 GiB of point records)
+    return b;
+  };
+  const int64_t budget_first = clamp_budget(n_points / 10 + 1), budget_rest = clamp_budget(n_points / 3 + 1);
   const int64_t kStarBudget = 1 << 20;
-  int64_t tf_sum = 0;
-  int64_t s0 = 0;
-  int64_t* row_tmp = nullptr;
-  while (s0 < n_stars) {
+  // sub-batch boundaries and the largest sub-batch
+  int64_t n_sub = 0, max_S = 0, max_np = 0;
+  for (int64_t s0 = 0; s0 < n_stars;) {
     int64_t s1 = s0 + 1;
-    while (s1 < n_stars && (row_ptr[s1 + 1] - row_ptr[s0]) <= kPointBudget && (s1 - s0) < kStarBudget) ++s1;
-    const int64_t S = s1 - s0, p0 = row_ptr[s0], np = row_ptr[s1] - p0;
-    if (np < 0) return QLP_BLS_EINVAL;
-    QLP_TRY(ctx->h_row.ensure((size_t)(S + 1) * 8));
-    QLP_TRY(ctx->h_t.ensure((size_t)(np + 1) * 8));
-    QLP_TRY(ctx->h_y.ensure((size_t)(np + 1) * 8));
-    QLP_TRY(ctx->h_dy.ensure((size_t)(np + 1) * 8));
-    QLP_TRY(ctx->h_rho.ensure((size_t)S * 8));
-    QLP_TRY(ctx->h_grid.ensure((size_t)S * sizeof(qlp_bls_star_grid)));
-    QLP_TRY(ctx->h_fptr.ensure((size_t)(S + 1) * 8));
-    QLP_TRY(ctx->h_peaks.ensure((size_t)S * K * sizeof(qlp_bls_peak)));
-    const int64_t* row_src = row_ptr + s0;
-    if (p0 != 0) {  // rebase the chunk's row_ptr to zero
-      row_tmp = (int64_t*)realloc(row_tmp, (size_t)(S + 1) * 8);
-      if (!row_tmp) return QLP_BLS_ENOMEM;
-      for (int64_t i = 0; i <= S; ++i) row_tmp[i] = row_ptr[s0 + i] - p0;
-      row_src = row_tmp;
+    const int64_t budget = s0 == 0 ? budget_first : budget_rest;
+    while (s1 < n_stars && (row_ptr[s1 + 1] - row_ptr[s0]) <= budget && (s1 - s0) < kStarBudget) ++s1;
+    if (s1 - s0 > max_S) max_S = s1 - s0;
+    if (row_ptr[s1] - row_ptr[s0] > max_np) max_np = row_ptr[s1] - row_ptr[s0];
+    if (row_ptr[s1] < row_ptr[s0]) return QLP_BLS_EINVAL;
+    ++n_sub; s0 = s1;
+  }
+  for (int i = 0; i < (n_sub > 1 ? 2 : 1); ++i) {
+    QLP_TRY(ctx->h_row[i].ensure((size_t)(max_S + 1) * 8));
+    QLP_TRY(ctx->h_t[i].ensure((size_t)(max_np + 1) * 8));
+    QLP_TRY(ctx->h_y[i].ensure((size_t)(max_np + 1) * 8));
+    QLP_TRY(ctx->h_dy[i].ensure((size_t)(max_np + 1) * 8));
+    QLP_TRY(ctx->h_rho[i].ensure((size_t)max_S * 8));
+  }
+  QLP_TRY(ctx->h_grid.ensure((size_t)max_S * sizeof(qlp_bls_star_grid)));
+  QLP_TRY(ctx->h_fptr.ensure((size_t)(max_S + 1) * 8));
+  QLP_TRY(ctx->h_peaks.ensure((size_t)max_S * K * sizeof(qlp_bls_peak)));
+  int64_t* row_tmp[2] = {nullptr, nullptr};
+  for (int i = 0; i < 2; ++i) {
+    row_tmp[i] = (int64_t*)malloc((size_t)(max_S + 1) * 8);
+    if (!row_tmp[i]) { free(row_tmp[0]); return QLP_BLS_ENOMEM; }
+  }
+  struct Sub { int64_t s0, s1; };
+  auto next_sub = [&](int64_t s0) {
+    int64_t s1 = s0 + 1;
+    const int64_t budget = s0 == 0 ? budget_first : budget_rest;
+    while (s1 < n_stars && (row_ptr[s1 + 1] - row_ptr[s0]) <= budget && (s1 - s0) < kStarBudget) ++s1;
+    return Sub{s0, s1};
+  };
+  // enqueue the H2D of one sub-batch on the copy stream into staging set `set`
+  auto issue_h2d = [&](const Sub& sb, int set, bool wait_free) -> int {
+    const int64_t S = sb.s1 - sb.s0, p0 = row_ptr[sb.s0], np = row_ptr[sb.s1] - p0;
+    cudaStream_t cs = ctx->copy_stream;
+    if (wait_free) CUDA_TRY(cudaStreamWaitEvent(cs, ctx->set_free[set], 0));
+    for (int64_t i = 0; i <= S; ++i) row_tmp[set][i] = row_ptr[sb.s0 + i] - p0;  // rebased to zero
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_row[set].p, row_tmp[set], (size_t)(S + 1) * 8, cudaMemcpyHostToDevice, cs));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_t[set].p, t + p0, (size_t)np * 8, cudaMemcpyHostToDevice, cs));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_y[set].p, y + p0, (size_t)np * 8, cudaMemcpyHostToDevice, cs));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_dy[set].p, dy + p0, (size_t)np * 8, cudaMemcpyHostToDevice, cs));
+    CUDA_TRY(cudaMemcpyAsync(ctx->h_rho[set].p, rho + sb.s0, (size_t)S * 8, cudaMemcpyHostToDevice, cs));
+    CUDA_TRY(cudaEventRecord(ctx->h2d_done[set], cs));
+    return 0;
+  };
+  int rc = 0;
+  int64_t tf_sum = 0;
+  Sub cur = next_sub(0);
+  rc = issue_h2d(cur, 0, false);
+  for (int64_t i = 0; rc == 0; ++i) {
+    const int set = (int)(i & 1);
+    const bool has_next = cur.s1 < n_stars;
+    Sub nxt = cur;
+    if (has_next) {
+      nxt = next_sub(cur.s1);
+      // the other set was last read by sub-batch i-1 (if any): its set_free event was recorded then
+      if ((rc = issue_h2d(nxt, set ^ 1, i >= 1)) != 0) break;
     }
-    CUDA_TRY(cudaMemcpyAsync(ctx->h_row.p, row_src, (size_t)(S + 1) * 8, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(ctx->h_t.p, t + p0, (size_t)np * 8, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(ctx->h_y.p, y + p0, (size_t)np * 8, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(ctx->h_dy.p, dy + p0, (size_t)np * 8, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(ctx->h_rho.p, rho + s0, (size_t)S * 8, cudaMemcpyHostToDevice, st));
-    if (row_src == row_tmp) CUDA_TRY(cudaStreamSynchronize(st));  // row_tmp is reused by the next chunk
+    const int64_t S = cur.s1 - cur.s0;
+    if (cudaStreamWaitEvent(st, ctx->h2d_done[set], 0) != cudaSuccess) { cudaGetLastError(); rc = QLP_BLS_ECUDA; break; }
+    const int64_t* d_row = (const int64_t*)ctx->h_row[set].p;
+    const double* d_t = (const double*)ctx->h_t[set].p;
+    const double* d_y = (const double*)ctx->h_y[set].p;
+    const double* d_dy = (const double*)ctx->h_dy[set].p;
     int64_t tf = 0, tb = 0;
-    ctx->last_row_ptr = nullptr;  // staging pointers are reused across chunks: never trust the cache
-    int rc = qlp_bls_grid(ctx, S, (const int64_t*)ctx->h_row.p, (const double*)ctx->h_t.p, (const double*)ctx->h_rho.p,
-                          nullptr, (qlp_bls_star_grid*)ctx->h_grid.p, (int64_t*)ctx->h_fptr.p, &tf, &tb, st);
-    if (rc != 0) { free(row_tmp); return rc; }
+    ctx->last_row_ptr = nullptr;  // staging pointers are reused across sub-batches: never trust the cache
+    rc = qlp_bls_grid(ctx, S, d_row, d_t, (const double*)ctx->h_rho[set].p, nullptr,
+                      (qlp_bls_star_grid*)ctx->h_grid.p, (int64_t*)ctx->h_fptr.p, &tf, &tb, st);
+    if (rc != 0) break;
     tf_sum += tf;
-    if ((rc = ctx->h_sr.ensure((size_t)(tf + 1) * 4)) != 0 || (rc = ctx->h_best.ensure((size_t)(tf + 1) * 4)) != 0) {
-      free(row_tmp); return rc;
-    }
-    rc = qlp_bls_spectrum(ctx, S, (const int64_t*)ctx->h_row.p, (const double*)ctx->h_t.p, (const double*)ctx->h_y.p,
-                          (const double*)ctx->h_dy.p, (const qlp_bls_star_grid*)ctx->h_grid.p,
+    if ((rc = ctx->h_sr.ensure((size_t)(tf + 1) * 4)) != 0 || (rc = ctx->h_best.ensure((size_t)(tf + 1) * 4)) != 0) break;
+    rc = qlp_bls_spectrum(ctx, S, d_row, d_t, d_y, d_dy, (const qlp_bls_star_grid*)ctx->h_grid.p,
                           (const int64_t*)ctx->h_fptr.p, (float*)ctx->h_sr.p, (uint32_t*)ctx->h_best.p, st);
     if (rc == 0)
-      rc = qlp_bls_snr(ctx, S, (const int64_t*)ctx->h_row.p, (const double*)ctx->h_t.p, (const double*)ctx->h_y.p,
-                       (const double*)ctx->h_dy.p, (const qlp_bls_star_grid*)ctx->h_grid.p,
+      rc = qlp_bls_snr(ctx, S, d_row, d_t, d_y, d_dy, (const qlp_bls_star_grid*)ctx->h_grid.p,
                        (const int64_t*)ctx->h_fptr.p, (const float*)ctx->h_sr.p, (const uint32_t*)ctx->h_best.p,
                        nullptr, (qlp_bls_peak*)ctx->h_peaks.p, st);
-    if (rc != 0) { free(row_tmp); return rc; }
-    cudaError_t e = cudaMemcpyAsync(peaks + s0 * K, ctx->h_peaks.p, (size_t)S * K * sizeof(qlp_bls_peak),
-                                    cudaMemcpyDeviceToHost, st);
+    if (rc != 0) break;
+    cudaError_t e = cudaEventRecord(ctx->set_free[set], st);
+    if (e == cudaSuccess)
+      e = cudaMemcpyAsync(peaks + cur.s0 * K, ctx->h_peaks.p, (size_t)S * K * sizeof(qlp_bls_peak),
+                          cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess && grid_out)
-      e = cudaMemcpyAsync(grid_out + s0, ctx->h_grid.p, (size_t)S * sizeof(qlp_bls_star_grid), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) { cudaGetLastError(); free(row_tmp); return QLP_BLS_ECUDA; }
-    s0 = s1;
+      e = cudaMemcpyAsync(grid_out + cur.s0, ctx->h_grid.p, (size_t)S * sizeof(qlp_bls_star_grid),
+                          cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) { cudaGetLastError(); rc = QLP_BLS_ECUDA; break; }
+    if (!has_next) break;
+    cur = nxt;
   }
-  free(row_tmp);
-  if (total_freq) *total_freq = tf_sum;
-  return QLP_BLS_OK;
+  // everything enqueued (or failed): drain both streams before the host buffers go out of scope
+  cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(ctx->copy_stream);
+  free(row_tmp[0]); free(row_tmp[1]);
+  if (rc == 0 && (e1 != cudaSuccess || e2 != cudaSuccess)) { cudaGetLastError(); rc = QLP_BLS_ECUDA; }
+  if (rc == 0 && total_freq) *total_freq = tf_sum;
+  return rc;
 }
 
 // ---- test-only entry points ---------------------------------------------------------------------------
