@@ -31,6 +31,10 @@ PEAK_DTYPE = np.dtype([("k", "i8"), ("freq", "f8"), ("period", "f8"), ("t0", "f8
                        ("nb", "i4"), ("status", "i4")], align=True)
 
 
+STATS_DTYPE = np.dtype([("n_in", "i4"), ("n_before", "i4"), ("n_after", "i4"), ("n_transits", "i4"),
+                        ("oot_level", "f8"), ("duration", "f8")], align=True)
+
+
 def default_config(**kw) -> Config:
     """PAPER.md:19 (0.5-2.0 x q_circ), :23 (a = 2 R*), :35 (samples_per_peak=2, dlogq=0.1, noverlap=3), :7 (27.4 d)."""
     c = Config(2.0, 0.1, 3, 0, 0.5, 2.0, 2.0, 27.4)
@@ -62,6 +66,7 @@ def lib():
         assert L.orc_sizeof_grid() == GRID_DTYPE.itemsize
         assert L.orc_sizeof_peak() == PEAK_DTYPE.itemsize
         assert L.orc_sizeof_config() == C.sizeof(Config)
+        assert L.orc_sizeof_peak_stats() == STATS_DTYPE.itemsize
         _lib = L
     return _lib
 
@@ -178,6 +183,15 @@ def peak_record(cfg: Config, g, t, y, dy, k: int, snr_k: float):
     lib().orc_peak_record(C.byref(cfg), _p(ga), C.c_int64(t.size), _p(t), _p(y), _p(dy),
                           C.c_int64(k), C.c_double(snr_k), _p(p))
     return p[0]
+
+
+def peak_statistics(t, y, dy, f: float, m: int, nb: int, t0: float):
+    """O7: points in / before / after transit, number of transits, out-of-transit level."""
+    t, y, dy = _f8(t), _f8(y), _f8(dy)
+    out = np.zeros(1, dtype=STATS_DTYPE)
+    lib().orc_peak_statistics(C.c_int64(t.size), _p(t), _p(y), _p(dy), C.c_double(f), C.c_int32(m), C.c_int32(nb),
+                              C.c_double(t0), _p(out))
+    return out[0]
 
 
 def batch(cfg: Config, row_ptr, t, y, dy, rho, K: int = 3, want_snr: bool = True, threads: int | None = None):

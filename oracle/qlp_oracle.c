@@ -427,3 +427,51 @@ int orc_batch(const orc_config* c, int64_t S, const int64_t* row_ptr, const doub
 int orc_sizeof_grid(void) { return (int)sizeof(orc_star_grid); }
 int orc_sizeof_peak(void) { return (int)sizeof(orc_peak); }
 int orc_sizeof_config(void) { return (int)sizeof(orc_config); }
+
+/* ---------------------------------------------------------------- O7 */
+/* "Other statistics" of a peak: "the number of points in, before, and after transit, number of
+ * transits, and out-of-transit magnitude level.  In order for a transit to count toward the number of
+ * transits, we require there to be data within 0.5 transit durations of the expected mid-transit time."
+ * Readings (O7): P = 1/f, duration D = q P with q = m/nb from the BLS; for every point
+ *   x = (t - T0)/P;  n = floor(x + 0.5);  dt = (x - n) P            (time from the nearest mid-transit)
+ *   in transit   : |dt| <= D/2            (this is also "data within 0.5 durations of the mid-time")
+ *   before/after : one duration wide, adjacent to the transit: -1.5 D <= dt < -D/2,  D/2 < dt <= 1.5 D
+ *   n_transits   : number of distinct n that own at least one in-transit point
+ *   oot level    : weighted mean (weights dy^-2) of y over the points that are not in transit.
+ * FP64, no FMA, operations in the order written (the classification is an integer decision). */
+typedef struct {
+  int32_t n_in, n_before, n_after, n_transits;
+  double oot_level, duration;
+} orc_peak_stats;
+
+void orc_peak_statistics(int64_t n, const double* t, const double* y, const double* dy, double f, int32_t m,
+                         int32_t nb, double t0, orc_peak_stats* out) {
+  double P = 1.0 / f;
+  double q = (double)m / (double)nb;
+  double D = q * P;
+  double hD = 0.5 * D, wD = 1.5 * D;
+  int32_t n_in = 0, n_before = 0, n_after = 0, n_tr = 0;
+  double sw = 0.0, swy = 0.0;
+  int have_prev = 0;
+  double prev_n = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    double x = (t[i] - t0) / P;
+    double cyc = floor(x + 0.5);
+    double dt = (x - cyc) * P;
+    int in = fabs(dt) <= hD;
+    if (in) {
+      ++n_in;
+      if (!have_prev || cyc != prev_n) ++n_tr;  /* t is increasing: in-transit points of one cycle are adjacent */
+      have_prev = 1; prev_n = cyc;
+    } else {
+      double w = 1.0 / (dy[i] * dy[i]);
+      sw += w; swy += w * y[i];
+      if (dt < -hD && dt >= -wD) ++n_before;
+      if (dt > hD && dt <= wD) ++n_after;
+    }
+  }
+  out->n_in = n_in; out->n_before = n_before; out->n_after = n_after; out->n_transits = n_tr;
+  out->oot_level = (sw > 0.0) ? swy / sw : 0.0;
+  out->duration = D;
+}
+int orc_sizeof_peak_stats(void) { return (int)sizeof(orc_peak_stats); }
