@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C] [--stars S]
 
-One "step" = one pass of the whole hot path (grid -> prep -> fold+box-scan -> S/N + peaks) over one
+One "step" = one pass of the whole hot path (grid -> prep -> fold+box-scan -> S/N + peaks -> peak statistics) over one
 batch.  Default workload = BASELINE.json configs[1] ("config 2": 1,000 stars, one sector at 200 s
 cadence, ~11.4k points and ~4.5k-10k frequencies per star).  Prints ONE JSON line (rank 0).
 
@@ -227,6 +227,7 @@ def run_gpu(args):
         grid, freq_ptr, tf, _ = ctx.grid(row_ptr, t, rho, rstar)
         sr, best = ctx.spectrum(row_ptr, t, y, dy, grid, freq_ptr, tf)
         _, peaks = ctx.snr(row_ptr, t, y, dy, grid, freq_ptr, sr, best, want_snr=False)
+        ctx.peak_stats(row_ptr, t, y, dy, peaks)  # O7, the first row after the search
         return grid, peaks, tf
 
     grid, peaks, tf = step()

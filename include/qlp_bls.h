@@ -102,6 +102,20 @@ typedef struct {
   int32_t status;  /* 0 = valid                                                                  */
 } qlp_bls_peak;
 
+/* "Other statistics" of one peak, written by qlp_bls_peak_stats() (device memory, [S * top_k],
+ * same order as the peak table).  DESIGN.md O7: a point is in transit when it lies within half a duration of the
+ * nearest expected mid-transit time T0 + n P, "before" / "after" are the one-duration-wide windows next to the
+ * transit, a transit counts only if it owns at least one in-transit point, and the out-of-transit level is the
+ * dy^-2-weighted mean of y over the points that are not in transit.  Invalid peaks give all zeros. */
+typedef struct {
+  int32_t n_in;        /* points in transit (n_t of PAPER.md Eq. 2)                                */
+  int32_t n_before;    /* points in [-1.5 D, -0.5 D) around the mid-times                          */
+  int32_t n_after;     /* points in (0.5 D, 1.5 D]                                                  */
+  int32_t n_transits;  /* transits with data within 0.5 D of the mid-time (N_t of PAPER.md Eq. 2)  */
+  double oot_level;    /* out-of-transit level, same unit as y                                     */
+  double duration;     /* D = (m / nb) * period, days                                              */
+} qlp_bls_transit_stats;
+
 /* Fill *cfg with the paper's defaults, device 0, top_k 3. */
 void qlp_bls_default_config(qlp_bls_config* cfg /*host*/);
 
@@ -139,6 +153,12 @@ int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const
                 const double* y, const double* dy, const qlp_bls_star_grid* grid,
                 const int64_t* freq_ptr, const float* sr, const uint32_t* best, float* snr,
                 qlp_bls_peak* peaks, void* cuda_stream);
+
+/* Per-peak statistics (O7; the row after the search in SURVEY.md 8(f)).
+ *   in : the batch (row_ptr, t, y, dy) and the peak table written by qlp_bls_snr, all dev.
+ *   out: stats dev [S * top_k]. */
+int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
+                       const double* dy, const qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, void* cuda_stream);
 
 /* Whole path with HOST buffers (pageable or pinned): copies the batch to the device, runs
  * grid -> spectrum -> snr, copies the peak table (and nothing else) back.  This is the call the

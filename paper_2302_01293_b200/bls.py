@@ -34,7 +34,10 @@ PEAK_DTYPE = np.dtype([("k", "i8"), ("freq", "f8"), ("period", "f8"), ("t0", "f8
                        ("snr", "f4"), ("q", "f4"), ("depth", "f4"), ("m", "i4"), ("j", "i4"),
                        ("nb", "i4"), ("status", "i4")], align=True)
 
-EXPORTS = ["qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
+STATS_DTYPE = np.dtype([("n_in", "i4"), ("n_before", "i4"), ("n_after", "i4"), ("n_transits", "i4"),
+                        ("oot_level", "f8"), ("duration", "f8")], align=True)
+
+EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
            "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
@@ -57,6 +60,7 @@ def load_library():
         L.qlp_bls_grid.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64), C.POINTER(i64), vp]
         L.qlp_bls_spectrum.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_snr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.qlp_bls_peak_stats.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_search_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
         L.qlp_bls_destroy.argtypes = [vp]
         L.qlp_bls_strerror.argtypes = [C.c_int]
@@ -196,6 +200,17 @@ class QlpBls:
                "qlp_bls_snr")
         return snr, peaks
 
+    # -- O7
+    def peak_stats(self, row_ptr, t, y, dy, peaks):
+        """qlp_bls_peak_stats -> stats uint8[S*top_k, 32] tensor (see stats_to_numpy)."""
+        torch = self.torch
+        S = int(row_ptr.numel()) - 1
+        stats = torch.zeros((max(S * self.top_k, 1), STATS_DTYPE.itemsize), dtype=torch.uint8,
+                            device=self.device)[:S * self.top_k]
+        _check(self.lib.qlp_bls_peak_stats(self._h, S, _ptr(row_ptr), _ptr(t), _ptr(y), _ptr(dy), _ptr(peaks),
+                                           _ptr(stats), self._stream()), "qlp_bls_peak_stats")
+        return stats
+
     # -- whole path from host (numpy / pinned torch CPU) buffers
     def search_host(self, row_ptr, t, y, dy, rho, want_grid: bool = False):
         """qlp_bls_search_host on numpy arrays -> (peaks structured [S, top_k], grid or None, total_freq)."""
@@ -245,6 +260,11 @@ def grid_to_numpy(grid_tensor) -> np.ndarray:
 
 def peaks_to_numpy(peaks_tensor, top_k: int) -> np.ndarray:
     a = np.frombuffer(peaks_tensor.cpu().numpy().tobytes(), dtype=PEAK_DTYPE).copy()
+    return a.reshape(-1, top_k)
+
+
+def stats_to_numpy(stats_tensor, top_k: int) -> np.ndarray:
+    a = np.frombuffer(stats_tensor.cpu().numpy().tobytes(), dtype=STATS_DTYPE).copy()
     return a.reshape(-1, top_k)
 
 

@@ -10,6 +10,7 @@
 #include "grid.cuh"
 #include "prep.cuh"
 #include "snr_kernel.cuh"
+#include "stats.cuh"
 
 using namespace qlp;
 
@@ -383,6 +384,20 @@ extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row
   snr_kernel<<<(unsigned)n_stars, kSnrThreads, kMaxSel * 256 * 4, st>>>(
       ctx->prm, n_stars, row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, grid, freq_ptr, sr, best,
       snr, peaks);
+  return launch_ok(ctx);
+}
+
+// ---- O7: per-peak statistics --------------------------------------------------------------------------
+extern "C" int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                  const double* y, const double* dy, const qlp_bls_peak* peaks,
+                                  qlp_bls_transit_stats* stats, void* cuda_stream) {
+  if (!ctx || n_stars < 0) return QLP_BLS_EINVAL;
+  if (n_stars == 0) return QLP_BLS_OK;
+  if (!row_ptr || !t || !y || !dy || !peaks || !stats) return QLP_BLS_EINVAL;
+  if (n_stars * ctx->prm.top_k > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  peak_stats_kernel<<<(unsigned)(n_stars * ctx->prm.top_k), 256, 0, (cudaStream_t)cuda_stream>>>(
+      n_stars, ctx->prm.top_k, row_ptr, t, y, dy, peaks, stats);
   return launch_ok(ctx);
 }
 
