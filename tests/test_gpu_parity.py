@@ -315,3 +315,32 @@ def test_constant_and_degenerate_light_curves(gpu, ctx, orc, cfg):
     for s in (1, 4):
         so = ob["sr"][fp[s]:fp[s + 1]]
         assert np.abs(sr[fp[s]:fp[s + 1]] - so).max() <= SR_RTOL * so.max()
+
+
+@pytest.mark.parametrize("kw", [dict(a_over_rstar_min=3.0),                       # Sectors 59-60 variant
+                                dict(noverlap=4, dlogq=0.2),                       # ladder {4,5,6,7,8,10,12,14}: gaps, width 14
+                                dict(noverlap=2, qmax_fac=3.0),                    # ladder {2..11}
+                                dict(noverlap=5, dlogq=0.05, qmax_fac=1.5)])       # ladder {5..15}
+def test_other_search_parameters(gpu, orc, kw):
+    """Non-default qlp_bls_config: grid bit-exact and SR parity with the oracle under the same parameters.
+    Ladders other than the paper's {3..11} run the generic (run-time mask, 16-wide window) kernel."""
+    from paper_2302_01293_b200 import synth
+    ocfg = orc.default_config(**kw)
+    b = synth.make_batch(2, n_stars=3)
+    ctx = gpu.QlpBls(**kw)
+    try:
+        assert ctx.widths().tolist() == orc.widths(ocfg).tolist()
+        dev = gpu.upload(b)
+        grid, freq_ptr, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        go = _oracle_grids(orc, ocfg, b)
+        _assert_grid_equal(gpu.grid_to_numpy(grid), go)
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, tf)
+        sr, best, fp = sr.cpu().numpy(), best.cpu().numpy(), freq_ptr.cpu().numpy()
+        ob = orc.batch(ocfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=0, want_snr=False)
+        for s in range(b.n_stars):
+            a, e = int(fp[s]), int(fp[s + 1])
+            rel, same, m_g, j_g = _compare_sr(sr[a:e], best[a:e], ob["sr"][a:e], ob["m"][a:e], ob["j"][a:e], f"{kw}[{s}]")
+            assert same > 0.98
+            assert set(np.unique(m_g)) <= set(orc.widths(ocfg).tolist())
+    finally:
+        ctx.close()
