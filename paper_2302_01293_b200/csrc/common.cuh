@@ -51,12 +51,6 @@ struct Params {
   int32_t min_width;  // smallest width (the all-zero answer, O4)
 };
 
-// One unit of work of the fold/scan kernel: `ncols` consecutive frequencies of one star.
-struct Tile {
-  int32_t star;
-  int32_t ncols;   // <= columns per CTA of the class
-  int64_t k0;      // first frequency index within the star
-};
 
 // ---- exact FP64 helpers: never contracted into FMAs (O1/O3: "no fused multiply-add") ---
 __device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a, b); }
