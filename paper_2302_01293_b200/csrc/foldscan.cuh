@@ -254,6 +254,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const int64_t n = ti.n_pts;
       const Point* src = pts + ti.pt_begin;
       const int64_t n_chunks = (n + kChunk - 1) / kChunk;
+      const bool swap_ws = (HPW > 1) && (hsub & 1);
+      const int first_off = swap_ws ? CTOT : 0;
       const uint32_t lane_off = (uint32_t)col0 * 4u;  // byte offset of this lane's first column in a row
       unsigned char* hbytes = reinterpret_cast<unsigned char*>(hist);
       __syncthreads();  // histograms zeroed
@@ -285,8 +287,16 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
               // low word = bin * (row bytes) + fraction bits: one LOP3 clears them and adds the lane
               const uint32_t off = (bin_offset_of<SB>(f[r], tau, dnb[r], K[r]) & ~((1u << SB) - 1u)) | lane_off;
               uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + 32 * r;
-              atomicAdd(cell, (uint32_t)v[u].z);
-              atomicAdd(cell + CTOT, (uint32_t)v[u].w);
+              if (HPW == 1) {
+                atomicAdd(cell, (uint32_t)v[u].z);
+                atomicAdd(cell + CTOT, (uint32_t)v[u].w);
+              } else {
+                // Narrow classes: the lanes that share a column fold different points, and with a row of
+                // 2*CTOT <= 32 words they would meet on one bank in both atomics.  Odd point-lanes therefore
+                // add S first and W second: in each instruction the two parities use different banks.
+                atomicAdd(cell + first_off, swap_ws ? (uint32_t)v[u].w : (uint32_t)v[u].z);
+                atomicAdd(cell + (CTOT - first_off), swap_ws ? (uint32_t)v[u].z : (uint32_t)v[u].w);
+              }
             }
           }
         }
