@@ -129,3 +129,33 @@ def test_bench_configuration_sampled(gpu, orc, cfg):
         assert len(deep) > 20 and hits >= 0.8 * len(deep), (hits, len(deep))
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("span", [0.6553, 0.66, 0.7, 0.8])
+def test_tiny_grids(gpu, orc, cfg, span):
+    """Baselines barely longer than 2 P_min: grids of one to a few dozen frequencies (Sturges N = 1, 2, ...)."""
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(4)
+    t = 100.0 + np.arange(0.0, span, 200.0 / 86400.0)
+    b = synth.from_arrays([(t, rng.standard_normal(t.size) * 1e-3, np.full(t.size, 1e-3))])
+    go = orc.grid(cfg, t, 1.0)
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        dev = gpu.upload(b)
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        assert gpu.grid_to_numpy(grid)[0].tobytes() == go.tobytes()
+        assert tf == int(go["n_freq"])
+        if tf == 0:
+            return
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        snr, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best)
+        ob = orc.batch(cfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=3, want_snr=True)
+        assert np.abs(sr.cpu().numpy() - ob["sr"]).max() <= SR_RTOL * ob["sr"].max()
+        scale = np.abs(ob["snr"]).max()
+        assert np.abs(snr.cpu().numpy() - ob["snr"]).max() <= 5e-4 * scale + 1e-3
+        pk = gpu.peaks_to_numpy(peaks, 3)
+        n_o = int((ob["peaks"][0]["k"] >= 0).sum())
+        assert int((pk[0]["k"] >= 0).sum()) == n_o
+        assert pk[0][0]["k"] == ob["peaks"][0][0]["k"] or abs(np.sort(ob["snr"])[-1] - np.sort(ob["snr"])[-2]) < 1e-3 * scale
+    finally:
+        ctx.close()
