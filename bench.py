@@ -63,6 +63,15 @@ def fold_issue_bound_evals_per_s(sm_mhz: float) -> float:
     return N_SM * sm_mhz * 1e6 * 4 * 32 / 11.25
 
 
+def scan_roofline(total_bins: int, n_widths: int, fold_s: float, scan_share: float, sm_mhz: float):
+    cand = float(total_bins) * n_widths
+    t = fold_s * scan_share
+    bound = N_SM * sm_mhz * 1e6 * 4 * 32 / 11.0  # 11 FP32/predicate instructions per candidate, one per clock
+    ach = cand / t if t > 0 else 0.0
+    return {"achieved": ach / 1e9, "peak": bound / 1e9, "unit": "Gcandidates/s", "frac": ach / bound,
+            "candidates_per_step": cand}
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -224,7 +233,8 @@ def run_gpu(args):
     S = batch.n_stars
 
     def step():
-        grid, freq_ptr, tf, _ = ctx.grid(row_ptr, t, rho, rstar)
+        grid, freq_ptr, tf, tb = ctx.grid(row_ptr, t, rho, rstar)
+        step.total_bins = tb
         sr, best = ctx.spectrum(row_ptr, t, y, dy, grid, freq_ptr, tf)
         _, peaks = ctx.snr(row_ptr, t, y, dy, grid, freq_ptr, sr, best, want_snr=False)
         ctx.peak_stats(row_ptr, t, y, dy, peaks)  # O7, the first row after the search
@@ -305,6 +315,10 @@ def run_gpu(args):
                      "phase_share": {"setup_zero": ph[0] / max(sum(ph), 1), "fold_S2": ph[1] / max(sum(ph), 1),
                                      "scan_S3": ph[2] / max(sum(ph), 1)},
                      "fold_only_achieved": achieved / 1e9 / max(ph[1] / max(sum(ph), 1), 1e-9),
+                     # S3 inside the fused kernel: (start bin, width) candidates per second over the scan's share of
+                     # the kernel time, against the FP32 issue bound of its 11-instruction candidate test
+                     "scan_S3": scan_roofline(step.total_bins, ctx.widths().size, fold_per_launch_s,
+                                              ph[2] / max(sum(ph), 1), sm_max),
                      "issue_bound": fold_issue_bound_evals_per_s(sm_max) / 1e9,
                      "frac_of_issue_bound": achieved / fold_issue_bound_evals_per_s(sm_max),
                      # dram__bytes_read+write of the foldscan launches of one step of THIS workload
