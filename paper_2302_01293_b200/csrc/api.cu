@@ -46,6 +46,10 @@ struct qlp_bls_ctx {
   DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev;
   // host-API staging
   DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks;
+  static const int kSide = 3;           // side streams for the independent tile-class launches
+  cudaStream_t side[kSide];
+  cudaEvent_t side_done[kSide], fork_ev;
+  bool fork_ready = false;
   cudaStream_t copy_stream = nullptr;  // H2D of the next sub-batch overlaps the search of the current one
   cudaEvent_t h2d_done[2], set_free[2];
   bool copy_ready = false;
@@ -169,6 +173,10 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks};
   for (DevBuf* b : bufs) b->release();
   if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
+  if (ctx->fork_ready) {
+    for (int i = 0; i < qlp_bls_ctx::kSide; ++i) { cudaStreamDestroy(ctx->side[i]); cudaEventDestroy(ctx->side_done[i]); }
+    cudaEventDestroy(ctx->fork_ev);
+  }
   if (ctx->copy_ready) {
     cudaStreamDestroy(ctx->copy_stream);
     for (int i = 0; i < 2; ++i) { cudaEventDestroy(ctx->h2d_done[i]); cudaEventDestroy(ctx->set_free[i]); }
@@ -343,7 +351,21 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   QLP_TRY(launch_ok(ctx));
   const int slot = (int)(ctx->ev_calls % qlp_bls_ctx::kRing);
   if (ctx->timing) CUDA_TRY(cudaEventRecord(ctx->ev0[slot], st));
+  // The class kernels are independent: they go to side streams so that the CTAs of the next class fill the SMs
+  // that the tail of the previous one leaves idle (each launch is persistent: any number of resident CTAs works).
+  if (!ctx->fork_ready) {
+    for (int i = 0; i < qlp_bls_ctx::kSide; ++i) {
+      CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
+      CUDA_TRY(cudaEventCreateWithFlags(&ctx->side_done[i], cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming));
+    ctx->fork_ready = true;
+  }
+  CUDA_TRY(cudaEventRecord(ctx->fork_ev, st));
+  for (int i = 0; i < qlp_bls_ctx::kSide; ++i) CUDA_TRY(cudaStreamWaitEvent(ctx->side[i], ctx->fork_ev, 0));
+  cudaStream_t user_st = st;
   for (int c = 0; c < kNumClasses; ++c) {
+    st = (c % (qlp_bls_ctx::kSide + 1) == 0) ? user_st : ctx->side[c % (qlp_bls_ctx::kSide + 1) - 1];
     const size_t smem = (size_t)class_smem_bytes(c);
     const int per_sm = class_ctas_per_sm(c);
     const unsigned nblk = (unsigned)(ctx->n_sm * per_sm);
@@ -365,6 +387,11 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
       default: QLP_LAUNCH_MW(1); break;
     }
     QLP_TRY(launch_ok(ctx));
+  }
+  st = user_st;
+  for (int i = 0; i < qlp_bls_ctx::kSide; ++i) {
+    CUDA_TRY(cudaEventRecord(ctx->side_done[i], ctx->side[i]));
+    CUDA_TRY(cudaStreamWaitEvent(st, ctx->side_done[i], 0));
   }
   if (ctx->timing) { CUDA_TRY(cudaEventRecord(ctx->ev1[slot], st)); ctx->ev_calls++; }
   return QLP_BLS_OK;
