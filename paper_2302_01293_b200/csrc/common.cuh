@@ -101,6 +101,23 @@ __device__ __forceinline__ int32_t bin_of(double f, double tau, double dnb, doub
   return __double2loint(v);
 }
 
+// The same bin from THREE FP64 instructions and integer arithmetic (what the fold kernel uses):
+//   I = floor(nb p)  = low word of RD(fma(p, nb, 2^52))      (exact: one rounding, downwards)
+//   g = floor(p)     = low word of RD(p + 2^52)
+//   floor(nb frac(p)) = I - nb g                              (nb g is an integer, so floor splits exactly)
+// The difference is below 2^15, so 32-bit wrap-around arithmetic on I and g is harmless.  The two FP64
+// results depend only on p, and the integer part folds into the address computation of the caller.
+__device__ __forceinline__ void bin_parts(double f, double tau, double dnb, uint32_t& I, uint32_t& g) {
+  const double p = __dmul_rn(f, tau);
+  I = (uint32_t)__double2loint(__fma_rd(p, dnb, QLP_TWO52));
+  g = (uint32_t)__double2loint(__dadd_rd(p, QLP_TWO52));
+}
+__device__ __forceinline__ int32_t bin_of3(double f, double tau, double dnb, uint32_t nb) {
+  uint32_t I, g;
+  bin_parts(f, tau, dnb, I, g);
+  return (int32_t)(I - nb * g);
+}
+
 // The same bin, delivered as a byte offset: with the magic constant 2^(52-SB) instead of 2^52 the
 // rounded-down sum has spacing 2^-SB, so the low word of v is floor(nb frac(p) 2^SB) = bin * 2^SB + (SB
 // fraction bits); the caller clears those with the same LOP3 that ORs in its lane offset.  Exact for the

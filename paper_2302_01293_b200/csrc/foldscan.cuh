@@ -241,7 +241,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     {
       // A column beyond the tile's last frequency folds with f = 0, nb = 1 into row 0 of its own
       // (never scanned) column: cheaper than predicating every atomic.
-      double f[R], dnb[R], K[R];
+      double f[R], dnb[R];
+      uint32_t neg_nb_row[R];  // -(nb * row bytes) mod 2^32
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         const int col = col0 + 32 * r;
@@ -249,7 +250,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         int32_t nbk = 1;
         if (col < ti.ncols) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
         dnb[r] = (double)nbk;
-        K[r] = bin_offset_K2<SB>(dnb[r]);
+        neg_nb_row[r] = 0u - (uint32_t)nbk * (uint32_t)(STRIDE * 4);
       }
       const int64_t n = ti.n_pts;
       const Point* src = pts + ti.pt_begin;
@@ -284,8 +285,10 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
             const double tau = __hiloint2double(v[u].y, v[u].x);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-              // low word = bin * (row bytes) + fraction bits: one LOP3 clears them and adds the lane
-              const uint32_t off = (bin_offset_of<SB>(f[r], tau, dnb[r], K[r]) & ~((1u << SB) - 1u)) | lane_off;
+              // byte offset of the bin's row: (I - nb g) * row bytes, as I * row + g * (-nb row) (+ lane)
+              uint32_t I, g;
+              bin_parts(f[r], tau, dnb[r], I, g);
+              const uint32_t off = g * neg_nb_row[r] + (I * (uint32_t)(STRIDE * 4) + lane_off);
               uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + 32 * r;
               if (HPW == 1) {
                 atomicAdd(cell, (uint32_t)v[u].z);

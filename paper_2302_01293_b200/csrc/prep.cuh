@@ -165,11 +165,10 @@ __global__ void debug_bins_kernel(Params prm, const int64_t* __restrict__ row_pt
   const qlp_bls_star_grid g = grid[star];
   double f; int32_t nb;
   freq_of_k(g.u0, g.h, dmul(prm.qmin_fac, g.c_q), (double)prm.noverlap, k, f, nb);
-  // the byte-offset form the fold kernel uses (row of 1024 bytes), shifted back to a bin number
-  const double dnb = (double)nb, K2 = bin_offset_K2<10>(dnb);
+  const double dnb = (double)nb;  // the three-instruction form the fold kernel uses
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     double tau = dsub(t[a + i], g.t_ref);
-    out[i] = (int32_t)(bin_offset_of<10>(f, tau, dnb, K2) >> 10);
+    out[i] = bin_of3(f, tau, dnb, (uint32_t)nb);
   }
 }
 
