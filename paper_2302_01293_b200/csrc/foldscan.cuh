@@ -117,6 +117,18 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
                    smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// Value s^2 / (r (1 - r)) of one box for the scan's running maximum, with O4's exclusions folded into the
+// arithmetic: d = r (c - r) with c = 1 - 2^-24 is negative for r >= 1 (the value then loses every fmaxf against
+// 0), and d = 0 only for r = 0, where s = 0 too and 0 * inf = NaN loses as well.  MUFU.RCP is within 1 ulp; the
+// relative change of d by c is 6e-8 / (1 - r).  Explicit _rn intrinsics: the same call gives the same bits.
+__device__ __forceinline__ float box_value(float r, float sm) {
+  const float t = __fadd_rn(0.99999994f, -r);
+  const float d = __fmul_rn(r, t);
+  float inv;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(d));
+  return __fmul_rn(__fmul_rn(sm, sm), inv);
+}
+
 struct TileInfo {
   int64_t k0, pt_begin, n_pts, out_base;
   double u0, h, Q;
@@ -318,11 +330,13 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     // ---- S3: box scan, in place ----
     // Each column is scanned by TPC threads, each over a contiguous range of start bins with the last
     // MW bins held in registers (statically indexed ring).  Window sums are formed left to right,
-    // exactly as O4 states them.  The running maximum is kept as a fraction (num, d) and updated with
-    // predicated moves: two multiplies and two compares per candidate, no division, no branch.
+    // exactly as O4 states them.  A candidate costs 8 instructions: two adds, box_value (FADD, 2 FMUL,
+    // MUFU.RCP, FMUL) and one FMNMX into the maximum of its start bin; the running maximum over start
+    // bins is updated once per start bin, and the width of the winner is recovered afterwards by
+    // re-evaluating that one start bin (same instructions, hence the same bits).
     constexpr int TPC = kThreads / CTOT;  // threads per column
     const int scol = tid % CTOT, seg = tid / CTOT;
-    float bnum = 0.f, bden = 1.f;  // running maximum as a fraction: no division in the scan
+    float bval = 0.f;
     uint32_t bidx = (uint32_t)prm.min_width << 24;
     const bool scol_on = scol < ti.ncols;
     int32_t nbk = 1;
@@ -336,6 +350,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const float inv_w = ti.inv_w;
       const uint32_t wmask = WM ? WM : prm.wmask;
       if (ja < jb) {
+        int bj = 0;
         float ww[MW], ss[MW];
 #pragma unroll
         for (int l = 0; l < MW - 1; ++l) {
@@ -354,29 +369,35 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
               if (e >= nbk) e -= nbk;
               ww[(jj + MW - 1) % MW] = (float)hc[e * STRIDE] * inv_w;
               ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * STRIDE + CTOT];
-              float r = 0.f, sm = 0.f;
+              float r = 0.f, sm = 0.f, vj = 0.f;
 #pragma unroll
               for (int m = 1; m <= MW; ++m) {
-                r += ww[(jj + m - 1) % MW];
-                sm += ss[(jj + m - 1) % MW];
-                if ((wmask >> m) & 1u) {
-                  const float d = fmaf(-r, r, r);  // r (1 - r)
-                  const float num = sm * sm;
-                  // branch-free running maximum of num/d by cross-multiplication (with 32 lanes a
-                  // warp-level "any lane improves" branch would be taken far too often)
-                  const bool up = (d > 0.f) && (num * bden > bnum * d);
-                  bnum = up ? num : bnum;
-                  bden = up ? d : bden;
-                  bidx = up ? (((uint32_t)m << 24) | (uint32_t)j) : bidx;
-                }
+                r = __fadd_rn(r, ww[(jj + m - 1) % MW]);
+                sm = __fadd_rn(sm, ss[(jj + m - 1) % MW]);
+                if ((wmask >> m) & 1u) vj = fmaxf(vj, box_value(r, sm));
               }
+              const bool up = vj > bval;  // strict: the earliest start bin keeps a tie
+              bval = up ? vj : bval;
+              bj = up ? j : bj;
             }
           }
+        }
+        if (bval > 0.f) {  // width of the winner: the narrowest one that reaches the maximum of its start bin
+          float r = 0.f, sm = 0.f;
+          int bm = 0;
+#pragma unroll 1
+          for (int m = 1; m <= MW; ++m) {
+            int e = bj + m - 1;
+            if (e >= nbk) e -= nbk;
+            r = __fadd_rn(r, (float)hc[e * STRIDE] * inv_w);
+            sm = __fadd_rn(sm, (float)(int32_t)hc[e * STRIDE + CTOT]);
+            if (((wmask >> m) & 1u) && bm == 0 && box_value(r, sm) == bval) bm = m;
+          }
+          bidx = ((uint32_t)bm << 24) | (uint32_t)bj;
         }
       }
     }
     // reduce over the TPC threads of a column (scratch = the idle staging buffers), earliest j wins ties
-    float bval = bnum / bden;
     float* cval = reinterpret_cast<float*>(pbuf);
     uint32_t* cidx = reinterpret_cast<uint32_t*>(pbuf) + kThreads;
     if (TPC > 1) {
