@@ -33,9 +33,9 @@ if ROOT not in sys.path:
 
 METRIC = "bls_point_frequency_evals_per_s"
 UNIT = "evals/s"
-# per evaluation the fold needs 2 shared-memory integer atomic lanes and 4 FP64
-# lanes; measured ceilings on B200 (profiles/ubench_r1.txt): ATOMS.ADD lanes/clk/SM and FP64
-# lanes/clk/SM.  The binding one is the atomic path.
+# per evaluation the fold needs 2 shared-memory integer atomic lanes and 3 FP64
+# lanes (the exact bin takes three FP64 instructions); measured ceilings on B200 (profiles/ubench_r1.txt):
+# ATOMS.ADD lanes/clk/SM and FP64 lanes/clk/SM.  The binding one is the atomic path.
 ATOMS_LANES_PER_CLK_SM = 31.6
 FP64_LANES_PER_CLK_SM = 62.3
 N_SM = 148
@@ -53,20 +53,21 @@ def _peaks():
 
 
 def fold_peak_evals_per_s(sm_mhz: float) -> float:
-    per_clk_sm = min(ATOMS_LANES_PER_CLK_SM / 2.0, FP64_LANES_PER_CLK_SM / 4.0)
+    per_clk_sm = min(ATOMS_LANES_PER_CLK_SM / 2.0, FP64_LANES_PER_CLK_SM / 3.0)
     return N_SM * sm_mhz * 1e6 * per_clk_sm
 
 
 def fold_issue_bound_evals_per_s(sm_mhz: float) -> float:
     """Tighter bound: an FP64 instruction costs its scheduler 2 issue cycles and nothing issues in its shadow
-    (profiles/ubench_r1.txt), so 32 evaluations cost >= 4*2 + 1 (address) + 2 (ATOMS) + 0.25 (LDS) cycles."""
-    return N_SM * sm_mhz * 1e6 * 4 * 32 / 11.25
+    (profiles/ubench_r1.txt), so 32 evaluations cost >= 3*2 + 2 (address) + 2 (ATOMS) + 0.25 (LDS) cycles."""
+    return N_SM * sm_mhz * 1e6 * 4 * 32 / 10.25
 
 
 def scan_roofline(total_bins: int, n_widths: int, fold_s: float, scan_share: float, sm_mhz: float):
     cand = float(total_bins) * n_widths
     t = fold_s * scan_share
-    bound = N_SM * sm_mhz * 1e6 * 4 * 32 / 11.0  # 11 FP32/predicate instructions per candidate, one per clock
+    # 8 instructions per candidate, one of them a MUFU.RCP (16 lanes/clk/SM): both give 16 candidates/clk/SM
+    bound = N_SM * sm_mhz * 1e6 * 16.0
     ach = cand / t if t > 0 else 0.0
     return {"achieved": ach / 1e9, "peak": bound / 1e9, "unit": "Gcandidates/s", "frac": ach / bound,
             "candidates_per_step": cand}
@@ -316,7 +317,7 @@ def run_gpu(args):
                                      "scan_S3": ph[2] / max(sum(ph), 1)},
                      "fold_only_achieved": achieved / 1e9 / max(ph[1] / max(sum(ph), 1), 1e-9),
                      # S3 inside the fused kernel: (start bin, width) candidates per second over the scan's share of
-                     # the kernel time, against the FP32 issue bound of its 11-instruction candidate test
+                     # the kernel time, against the issue / MUFU bound of its 8-instruction candidate test
                      "scan_S3": scan_roofline(step.total_bins, ctx.widths().size, fold_per_launch_s,
                                               ph[2] / max(sum(ph), 1), sm_max),
                      "issue_bound": fold_issue_bound_evals_per_s(sm_max) / 1e9,
@@ -327,7 +328,7 @@ def run_gpu(args):
                      "traffic_unit": "bytes per step (ncu dram read+write over the foldscan launches); algorithmic: "
                                      f"{4 * 16 * int(batch.n_points) + 8 * int(tf)} (points read once per tile class + SR/best)",
                      "share_of_step": fold_ms / max(n_timed, 1) / (ms / args.steps),
-                     "peak_source": f"148 SMs x {sm_max:.0f} MHz ({src}) x min(ATOMS lanes/2, FP64 lanes/4) per clk "
+                     "peak_source": f"148 SMs x {sm_max:.0f} MHz ({src}) x min(ATOMS lanes/2, FP64 lanes/3) per clk "
                                     "(profiles/ubench_r1.txt; DESIGN.md Roofline)"},
     }
     if world == 1 and not args.no_cpu:
