@@ -118,23 +118,6 @@ __device__ __forceinline__ int32_t bin_of3(double f, double tau, double dnb, uin
   return (int32_t)(I - nb * g);
 }
 
-// The same bin, delivered as a byte offset: with the magic constant 2^(52-SB) instead of 2^52 the
-// rounded-down sum has spacing 2^-SB, so the low word of v is floor(nb frac(p) 2^SB) = bin * 2^SB + (SB
-// fraction bits); the caller clears those with the same LOP3 that ORs in its lane offset.  Exact for the
-// same reason as bin_of (floor(floor(x 2^SB) / 2^SB) = floor(x)).  K2 = nb * 2^52 + 2^(52-SB).
-template <int SB>
-__device__ __forceinline__ uint32_t bin_offset_of(double f, double tau, double dnb, double K2) {
-  double p = __dmul_rn(f, tau);
-  double c = __dadd_rd(p, QLP_TWO52);
-  double A = __fma_rn(-dnb, c, K2);
-  double v = __fma_rd(p, dnb, A);
-  return (uint32_t)__double2loint(v);
-}
-template <int SB>
-__device__ __forceinline__ double bin_offset_K2(double dnb) {
-  return __fma_rn(dnb, QLP_TWO52, (double)(1ull << (52 - SB)));
-}
-
 // Tile classes of the fold/scan kernel: columns per CTA and the largest nb the class holds.
 // shared memory = cols * nbcap * 8 bytes of histograms + kStageBytes of point staging; class 0 fits
 // two CTAs per SM, the others one.

@@ -161,9 +161,6 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
   __shared__ TileInfo ti;
   __shared__ int64_t s_tile;
   constexpr int STRIDE = 2 * CTOT;              // words per histogram row: [W x CTOT][S x CTOT]
-  constexpr int SB = (CTOT == 128) ? 10 : (CTOT == 64) ? 9 : (CTOT == 32) ? 8 : (CTOT == 16) ? 7 :
-                     (CTOT == 8) ? 6 : (CTOT == 4) ? 5 : (CTOT == 2) ? 4 : 3;  // log2(row bytes)
-  static_assert((1 << SB) == STRIDE * 4, "row bytes must be a power of two");
   constexpr int CW = CTOT < 32 ? CTOT : 32;     // distinct columns across the lanes of a warp
   constexpr int R = CTOT / CW;                  // columns per lane
   constexpr int HPW = 32 / CW;                  // points per warp iteration
