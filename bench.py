@@ -275,15 +275,15 @@ def run_gpu(args):
     # end to end through the host-buffer API: pinned host inputs, H2D and D2H inside the timed region
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     h = [pin(batch.row_ptr), pin(batch.t), pin(batch.y), pin(batch.dy), pin(batch.rho)]
-    ctx.search_host(*h)
+    ctx.search_host(*h, want_stats=True)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        pk_host, _, _ = ctx.search_host(*h)
+        pk_host, st_host, _, _ = ctx.search_host(*h, want_stats=True)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     h2d = int(sum(a.nbytes for a in h))
-    d2h = int(pk_host.nbytes)
+    d2h = int(pk_host.nbytes + st_host.nbytes)
 
     ms, e2e_ms, evals_all, stars_all = aggregate_over_ranks(ms, e2e_s * 1e3, evals, S, world, f"cuda:{local}")
     if rank != 0:

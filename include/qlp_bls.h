@@ -160,13 +160,14 @@ int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const
 int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
                        const double* dy, const qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, void* cuda_stream);
 
-/* Whole path with HOST buffers (pageable or pinned): copies the batch to the device, runs
- * grid -> spectrum -> snr, copies the peak table (and nothing else) back.  This is the call the
- * end-to-end benchmark times.  peaks host [S * top_k]; grid_out host [S] or NULL. */
+/* Whole path with HOST buffers (pageable or pinned): copies the batch to the device in sub-batches (the copy of
+ * the next one overlaps the search of the current one), runs grid -> spectrum -> snr (-> peak_stats), copies the
+ * peak table (and the statistics) back.  This is the call the end-to-end benchmark times.
+ * peaks host [S * top_k]; stats host [S * top_k] or NULL; grid_out host [S] or NULL; total_freq host or NULL. */
 int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                         const double* y, const double* dy, const double* rho, const double* rstar,
-                        qlp_bls_peak* peaks, qlp_bls_star_grid* grid_out, int64_t* total_freq,
-                        void* cuda_stream);
+                        qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_star_grid* grid_out,
+                        int64_t* total_freq, void* cuda_stream);
 
 /* Release the context and its workspace.  NULL is allowed. */
 int qlp_bls_destroy(qlp_bls_ctx* ctx);

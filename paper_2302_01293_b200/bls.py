@@ -61,7 +61,7 @@ def load_library():
         L.qlp_bls_spectrum.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_snr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_peak_stats.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
-        L.qlp_bls_search_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
+        L.qlp_bls_search_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
         L.qlp_bls_destroy.argtypes = [vp]
         L.qlp_bls_strerror.argtypes = [C.c_int]
         L.qlp_bls_strerror.restype = C.c_char_p
@@ -212,18 +212,23 @@ class QlpBls:
         return stats
 
     # -- whole path from host (numpy / pinned torch CPU) buffers
-    def search_host(self, row_ptr, t, y, dy, rho, want_grid: bool = False):
-        """qlp_bls_search_host on numpy arrays -> (peaks structured [S, top_k], grid or None, total_freq)."""
+    def search_host(self, row_ptr, t, y, dy, rho, want_grid: bool = False, want_stats: bool = False):
+        """qlp_bls_search_host on numpy arrays -> (peaks structured [S, top_k], grid or None, total_freq)
+        or, with want_stats, (peaks, stats [S, top_k], grid or None, total_freq)."""
         S = int(row_ptr.shape[0]) - 1
         peaks = np.zeros(S * self.top_k, dtype=PEAK_DTYPE)
+        stats = np.zeros(S * self.top_k, dtype=STATS_DTYPE) if want_stats else None
         grid = np.zeros(S, dtype=GRID_DTYPE) if want_grid else None
         tf = C.c_int64()
 
         def hp(a):
             return C.c_void_p(a.ctypes.data)
         _check(self.lib.qlp_bls_search_host(self._h, S, hp(row_ptr), hp(t), hp(y), hp(dy), hp(rho), None, hp(peaks),
-                                            hp(grid) if want_grid else None, C.byref(tf), self._stream()),
+                                            hp(stats) if want_stats else None, hp(grid) if want_grid else None,
+                                            C.byref(tf), self._stream()),
                "qlp_bls_search_host")
+        if want_stats:
+            return peaks.reshape(S, self.top_k), stats.reshape(S, self.top_k), grid, int(tf.value)
         return peaks.reshape(S, self.top_k), grid, int(tf.value)
 
     # -- test-only

@@ -45,7 +45,7 @@ struct qlp_bls_ctx {
   // workspace
   DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev;
   // host-API staging
-  DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks;
+  DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats;
   static const int kSide = 3;           // side streams for the independent tile-class launches
   cudaStream_t side[kSide];
   cudaEvent_t side_done[kSide], fork_ev;
@@ -170,7 +170,7 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
                     &ctx->totals_dev, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
                     &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
-                    &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks};
+                    &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats};
   for (DevBuf* b : bufs) b->release();
   if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
   if (ctx->fork_ready) {
@@ -437,8 +437,8 @@ extern "C" int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64
 // small next to 180 GB of HBM.
 extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                    const double* y, const double* dy, const double* rho, const double* rstar,
-                                   qlp_bls_peak* peaks, qlp_bls_star_grid* grid_out, int64_t* total_freq,
-                                   void* cuda_stream) {
+                                   qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_star_grid* grid_out,
+                                   int64_t* total_freq, void* cuda_stream) {
   (void)rstar;
   if (!ctx || n_stars < 0 || !row_ptr || !peaks) return QLP_BLS_EINVAL;
   if (n_stars > 0 && (!t || !y || !dy || !rho)) return QLP_BLS_EINVAL;
@@ -487,6 +487,7 @@ extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int6
   QLP_TRY(ctx->h_grid.ensure((size_t)max_S * sizeof(qlp_bls_star_grid)));
   QLP_TRY(ctx->h_fptr.ensure((size_t)(max_S + 1) * 8));
   QLP_TRY(ctx->h_peaks.ensure((size_t)max_S * K * sizeof(qlp_bls_peak)));
+  if (stats) QLP_TRY(ctx->h_stats.ensure((size_t)max_S * K * sizeof(qlp_bls_transit_stats)));
   int64_t* row_tmp[2] = {nullptr, nullptr};
   for (int i = 0; i < 2; ++i) {
     row_tmp[i] = (int64_t*)malloc((size_t)(max_S + 1) * 8);
@@ -545,8 +546,14 @@ extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int6
       rc = qlp_bls_snr(ctx, S, d_row, d_t, d_y, d_dy, (const qlp_bls_star_grid*)ctx->h_grid.p,
                        (const int64_t*)ctx->h_fptr.p, (const float*)ctx->h_sr.p, (const uint32_t*)ctx->h_best.p,
                        nullptr, (qlp_bls_peak*)ctx->h_peaks.p, st);
+    if (rc == 0 && stats)
+      rc = qlp_bls_peak_stats(ctx, S, d_row, d_t, d_y, d_dy, (const qlp_bls_peak*)ctx->h_peaks.p,
+                              (qlp_bls_transit_stats*)ctx->h_stats.p, st);
     if (rc != 0) break;
     cudaError_t e = cudaEventRecord(ctx->set_free[set], st);
+    if (e == cudaSuccess && stats)
+      e = cudaMemcpyAsync(stats + cur.s0 * K, ctx->h_stats.p, (size_t)S * K * sizeof(qlp_bls_transit_stats),
+                          cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess)
       e = cudaMemcpyAsync(peaks + cur.s0 * K, ctx->h_peaks.p, (size_t)S * K * sizeof(qlp_bls_peak),
                           cudaMemcpyDeviceToHost, st);

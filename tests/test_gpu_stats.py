@@ -29,6 +29,8 @@ def test_peak_stats_match_oracle(gpu, orc, config, ids):
         _, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best, want_snr=False)
         stats = gpu.stats_to_numpy(ctx.peak_stats(dev[0], dev[1], dev[2], dev[3], peaks), ctx.top_k)
         pk = gpu.peaks_to_numpy(peaks, ctx.top_k)
+        pk_h, st_h, _, _ = ctx.search_host(b.row_ptr, b.t, b.y, b.dy, b.rho, want_stats=True)  # host path: same bits
+        assert pk_h.tobytes() == pk.tobytes() and st_h.tobytes() == stats.tobytes()
         checked = 0
         for s in range(b.n_stars):
             t, y, dy = b.star(s)
