@@ -190,7 +190,7 @@ def run_reference(args):
                             "sample": f"{n} stars per step, {args.steps} steps"},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
-    print(json.dumps(out))
+    emit(json.dumps(out))
 
 
 def shard_star_ids(n_stars_per_gpu: int, rank: int) -> np.ndarray:
@@ -219,11 +219,12 @@ def run_gpu(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the QLP BLS path has no CPU fallback)")
-    if world > 1:
+    use_dist = world > 1 or os.environ.get("QLP_BENCH_FORCE_DIST") == "1"  # the latter: exercise NCCL at world 1
+    if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
         build.build()
-    if world > 1:
+    if use_dist:
         dist.barrier()
     torch.cuda.set_device(local)
     ctx = bls.QlpBls(device=local, top_k=3)
@@ -249,7 +250,7 @@ def run_gpu(args):
     torch.cuda.synchronize()
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -285,9 +286,10 @@ def run_gpu(args):
     h2d = int(sum(a.nbytes for a in h))
     d2h = int(pk_host.nbytes + st_host.nbytes)
 
-    ms, e2e_ms, evals_all, stars_all = aggregate_over_ranks(ms, e2e_s * 1e3, evals, S, world, f"cuda:{local}")
+    ms, e2e_ms, evals_all, stars_all = aggregate_over_ranks(ms, e2e_s * 1e3, evals, S, 2 if use_dist else 1,
+                                                            f"cuda:{local}")
     if rank != 0:
-        if world > 1:
+        if use_dist:
             dist.destroy_process_group()
         return
     peaks_info, src = _peaks()
@@ -333,9 +335,27 @@ def run_gpu(args):
     }
     if world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(batch)
-    print(json.dumps(out))
-    if world > 1:
+    emit(json.dumps(out))
+    if use_dist:
         dist.destroy_process_group()
+
+
+_REAL_STDOUT = None
+
+
+def _quiet_stdout():
+    """Libraries (NCCL prints its version line) may write to stdout; the driver wants exactly one JSON line there.
+    File descriptor 1 is pointed at stderr for the run and the JSON line goes to the saved descriptor."""
+    global _REAL_STDOUT
+    sys.stdout.flush()
+    _REAL_STDOUT = os.fdopen(os.dup(1), "w")
+    os.dup2(2, 1)
+
+
+def emit(line: str):
+    out = _REAL_STDOUT or sys.stdout
+    out.write(line + "\n")
+    out.flush()
 
 
 def main():
@@ -349,6 +369,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    _quiet_stdout()
     if args.impl == "reference":
         run_reference(args)
     else:
