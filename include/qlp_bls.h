@@ -48,6 +48,10 @@ enum qlp_bls_status {
  * one SM's shared memory; reading A16).  Not reached for rho* <= 30, P <= 180 d. */
 #define QLP_BLS_MAX_NB 24576
 
+/* Largest number of points per star (the 32-bit fixed-point weights of the shared-memory histograms must not
+ * overflow when every point of a star lands in one bin).  Longer light curves are skipped with status 5. */
+#define QLP_BLS_MAX_POINTS 4194304
+
 /* Search parameters.  POD, caller-owned, copied by qlp_bls_create().  Defaults = the paper's. */
 typedef struct {
   uint32_t struct_bytes;    /* = sizeof(qlp_bls_config), for versioning                          */
@@ -81,7 +85,8 @@ typedef struct {
   int64_t n_freq;   /* number of trial frequencies                                               */
   int32_t nb_max;   /* phase bins at k = 0 (the largest)                                         */
   int32_t status;   /* 0 ok; 1 fewer than 2 points; 2 baseline <= 0; 3 f_max <= f_min;
-                       4 nb_max > QLP_BLS_MAX_NB (star skipped, n_freq = 0)                      */
+                       4 nb_max > QLP_BLS_MAX_NB (star skipped, n_freq = 0);
+                       5 more than QLP_BLS_MAX_POINTS points (star skipped, n_freq = 0)           */
 } qlp_bls_star_grid;
 
 /* One peak of one star, written by qlp_bls_snr() (device memory, [S * top_k], rank-major within

@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(256) grid_kernel(Params prm, int64_t n_stars, 
           double qlo = dmul(Q, dmul(u0, u0));
           q.nb_max = (int32_t)ceil(ddiv((double)prm.noverlap, qlo));
           if (q.nb_max > QLP_BLS_MAX_NB || q.nb_max <= 0) { q.status = 4; q.n_freq = 0; }
+          else if (n >= (int64_t)QLP_BLS_MAX_POINTS) { q.status = 5; q.n_freq = 0; }  // fixed-point weights
         }
       }
     }

@@ -159,3 +159,25 @@ def test_tiny_grids(gpu, orc, cfg, span):
         assert pk[0][0]["k"] == ob["peaks"][0][0]["k"] or abs(np.sort(ob["snr"])[-1] - np.sort(ob["snr"])[-2]) < 1e-3 * scale
     finally:
         ctx.close()
+
+
+def test_star_above_point_cap_is_skipped(gpu):
+    """QLP_BLS_MAX_POINTS = 2^22 points per star (32-bit fixed-point weights): longer series get status 5."""
+    from paper_2302_01293_b200 import synth
+    n = 1 << 22
+    t_big = 100.0 + np.arange(n, dtype=np.float64) * 1e-4
+    t_ok = synth.sector_times(0, 1800.0)
+    rng = np.random.default_rng(6)
+    b = synth.from_arrays([(t_big, np.zeros(n), np.ones(n)), (t_ok, rng.standard_normal(t_ok.size), np.ones(t_ok.size))])
+    ctx = gpu.QlpBls()
+    try:
+        dev = gpu.upload(b)
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        g = gpu.grid_to_numpy(grid)
+        assert g["status"].tolist() == [5, 0] and g["n_freq"][0] == 0 and g["n_freq"][1] > 0
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        _, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best, want_snr=False)
+        pk = gpu.peaks_to_numpy(peaks, ctx.top_k)
+        assert pk[0][0]["k"] == -1 and pk[1][0]["k"] >= 0
+    finally:
+        ctx.close()
