@@ -379,19 +379,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
             }
           }
         }
-        if (bval > 0.f) {  // width of the winner: the narrowest one that reaches the maximum of its start bin
-          float r = 0.f, sm = 0.f;
-          int bm = 0;
-#pragma unroll 1
-          for (int m = 1; m <= MW; ++m) {
-            int e = bj + m - 1;
-            if (e >= nbk) e -= nbk;
-            r = __fadd_rn(r, (float)hc[e * STRIDE] * inv_w);
-            sm = __fadd_rn(sm, (float)(int32_t)hc[e * STRIDE + CTOT]);
-            if (((wmask >> m) & 1u) && bm == 0 && box_value(r, sm) == bval) bm = m;
-          }
-          bidx = ((uint32_t)bm << 24) | (uint32_t)bj;
-        }
+        bidx = (uint32_t)bj;  // the width is recovered after the reduction, by one thread per column
       }
     }
     // reduce over the TPC threads of a column (scratch = the idle staging buffers), earliest j wins ties
@@ -406,8 +394,25 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         const float v = cval[g2 * CTOT + scol];
         if (v > bval) { bval = v; bidx = cidx[g2 * CTOT + scol]; }
       }
-      int bm = (int)(bidx >> 24), bj = (int)(bidx & 0xffffffu);
+      int bm = prm.min_width, bj = 0;
       if (bval > 0.f) {
+        // width of the winner: the narrowest one that reaches the maximum of its start bin (same
+        // instructions as in the scan, hence the same bits)
+        bj = (int)(bidx & 0xffffffu);
+        {
+          const uint32_t* hcw = hist + scol;
+          const uint32_t wmask = WM ? WM : prm.wmask;
+          float r = 0.f, sm = 0.f;
+          bm = 0;
+#pragma unroll 1
+          for (int m = 1; m <= MW; ++m) {
+            int e = bj + m - 1;
+            if (e >= nbk) e -= nbk;
+            r = __fadd_rn(r, (float)hcw[e * STRIDE] * ti.inv_w);
+            sm = __fadd_rn(sm, (float)(int32_t)hcw[e * STRIDE + CTOT]);
+            if (((wmask >> m) & 1u) && bm == 0 && box_value(r, sm) == bval) bm = m;
+          }
+        }
         // Canonical representative of the winning box (O4 ties: smaller m, then smaller j).  Boxes
         // that hold the same points have the same value; trim the empty bins off both ends, then
         // take the narrowest ladder width that still covers the occupied span and, for it, the
