@@ -142,15 +142,20 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
   }
   ctx->n_sm = n_sm;
-  int max_smem = 0;  // largest class: 231,440 B (+ static) <= 227 KB
-  for (int c = 0; c < kNumClasses; ++c) max_smem = class_smem_bytes(c) > max_smem ? class_smem_bytes(c) : max_smem;
+  // each instantiation gets the dynamic shared memory of the largest class that uses it
+  auto smem_for_cols = [](int cols) {
+    int m = 0;
+    for (int c = 0; c < kNumClasses; ++c)
+      if (class_cols(c) == cols && class_smem_bytes(c) > m) m = class_smem_bytes(c);
+    return m;
+  };
   bool attr_ok = true;
 #define QLP_ATTR(CT_)                                                                                                \
   attr_ok = attr_ok &&                                                                                               \
-            cudaFuncSetAttribute(foldscan_kernel<11, CT_, kPaperMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
-                cudaSuccess &&                                                                                       \
-            cudaFuncSetAttribute(foldscan_kernel<16, CT_, 0u>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem) == \
-                cudaSuccess
+            cudaFuncSetAttribute(foldscan_kernel<11, CT_, kPaperMask>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                                 smem_for_cols(CT_)) == cudaSuccess &&                                               \
+            cudaFuncSetAttribute(foldscan_kernel<16, CT_, 0u>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
+                                 smem_for_cols(CT_)) == cudaSuccess
   QLP_ATTR(128); QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
   if (!attr_ok ||
       cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
