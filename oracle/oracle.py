@@ -194,6 +194,21 @@ def peak_statistics(t, y, dy, f: float, m: int, nb: int, t0: float):
     return out[0]
 
 
+TRAP_DTYPE = np.dtype([("t0", "f8"), ("depth", "f8"), ("q", "f8"), ("q_in", "f8"), ("z", "f8"), ("chi2", "f8"),
+                       ("chi2_init", "f8"), ("n_fit", "i4"), ("n_eval", "i4"), ("status", "i4"), ("pad_", "i4")],
+                      align=True)
+
+
+def trapezoid_fit(t, y, dy, f: float, m: int, nb: int, t0: float):
+    """O8: trapezoid fit (T0, depth, q, q_in, z) of one peak at fixed P = 1/f."""
+    t, y, dy = _f8(t), _f8(y), _f8(dy)
+    out = np.zeros(1, dtype=TRAP_DTYPE)
+    assert lib().orc_sizeof_trapezoid() == TRAP_DTYPE.itemsize
+    lib().orc_trapezoid_fit(C.c_int64(t.size), _p(t), _p(y), _p(dy), C.c_double(f), C.c_int32(m), C.c_int32(nb),
+                            C.c_double(t0), _p(out))
+    return out[0]
+
+
 def batch(cfg: Config, row_ptr, t, y, dy, rho, K: int = 3, want_snr: bool = True, threads: int | None = None):
     """Whole path on a CSR batch (OpenMP over stars) -> dict(grid, freq_ptr, sr, m, j, snr, peaks)."""
     row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)

@@ -19,6 +19,7 @@
  *   O2 prep (Kovacs et al. 2002 weights)
  *   O3 bin index                O4 box scan -> SR(f), best (m, j)
  *   O5 S/N spectrum (footnote 3 at :65)   O6 peaks
+ *   O7 per-peak statistics                  O8 trapezoid fit
  */
 #include <math.h>
 #include <stdint.h>
@@ -475,3 +476,117 @@ void orc_peak_statistics(int64_t n, const double* t, const double* y, const doub
   out->duration = D;
 }
 int orc_sizeof_peak_stats(void) { return (int)sizeof(orc_peak_stats); }
+
+/* ---------------------------------------------------------------- O8 */
+/* Trapezoid model fit of one peak: "a trapezoid model parameterized by the orbital period (P),
+ * transit epoch (T0), depth (delta), duration divided by orbital period (q), duration of ingress divided by
+ * transit duration (q_in), and out-of-transit magnitude level (z).  P is fixed to the BLS period while other
+ * parameters are fit using initial guesses from BLS.  To speed up the fit, we only fit data within two transit
+ * durations of the transit center.  We place bounds on q between 0 and 1, and q_in between 0 (perfectly
+ * box-shaped) and 0.5 (V-shaped)."  The paper names no optimiser; readings (O8):
+ *   data     : P = 1/f, q0 = m/nb, D0 = q0 P; x = (t - T0_bls)/P; n = floor(x + 0.5); dt = (x - n) P (as O7);
+ *              the points with |dt| <= 2 D0 are the data of the fit, fixed for the whole fit; w = dy^-2.
+ *   model    : y ~ z - delta * sh(|dt - c|), c = T0 - T0_bls, D = q P, half = D/2, ing = q_in D,
+ *              sh(u) = 0 for u >= half, (half - u)/ing for half - u < ing, else 1   (delta > 0 is a dip, as O6).
+ *   linear   : for given (c, q, q_in), z and delta are the weighted least-squares solution (they enter
+ *              linearly); chi2 = sum w (y - model)^2 with that solution.  If the weighted variance of sh is
+ *              below 1e-9 (no point, or every point, at one level) delta = 0, z = weighted mean.
+ *   search   : compass search over (c, q, q_in) from (0, q0, 0.25) with steps (D0/4, q0/4, 0.125), bounds
+ *              c in [-D0, D0], q in [0, 1], q_in in [0, 0.5]: sweep the six moves (+,- per coordinate, in
+ *              that order), accept a move iff chi2 strictly decreases; when a sweep accepts nothing halve the
+ *              steps; 24 halvings; at most 600 evaluations.
+ * FP64; the sums run over the selected points in time order. */
+typedef struct {
+  double t0, depth, q, q_in, z, chi2, chi2_init;
+  int32_t n_fit, n_eval, status, pad_;
+} orc_trapezoid;
+
+typedef struct { int64_t n; const double *dt, *yt, *w; double A, ybar, G, P; } orc_fit_data;
+
+static double orc_trap_shape(double u, double half, double ing) {
+  if (u >= half) return 0.0;
+  double d = half - u;
+  if (d < ing) return d / ing;
+  return 1.0;
+}
+
+/* chi2 at (c, q, q_in); also the linear solution (delta, z). */
+static double orc_trap_chi2(const orc_fit_data* fd, double c, double q, double qin, double* delta, double* z) {
+  double D = q * fd->P, half = 0.5 * D, ing = qin * D;
+  double B = 0.0, Cc = 0.0, F = 0.0;
+  for (int64_t i = 0; i < fd->n; ++i) {
+    double sh = orc_trap_shape(fabs(fd->dt[i] - c), half, ing);
+    double wsh = fd->w[i] * sh;
+    B += wsh; Cc += wsh * sh; F += wsh * fd->yt[i];
+  }
+  double V = Cc - B * B / fd->A;          /* A times the weighted variance of sh */
+  double dl = 0.0;
+  if (V > 1e-9 * fd->A) dl = -F / V;      /* yt is centred: sum w yt = 0 */
+  double zc = dl * B / fd->A;             /* z - ybar */
+  double chi2 = 0.0;
+  for (int64_t i = 0; i < fd->n; ++i) {
+    double sh = orc_trap_shape(fabs(fd->dt[i] - c), half, ing);
+    double r = fd->yt[i] - zc + dl * sh;
+    chi2 += fd->w[i] * r * r;
+  }
+  *delta = dl; *z = fd->ybar + zc;
+  return chi2;
+}
+
+void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double* dy, double f, int32_t m,
+                       int32_t nb, double t0_bls, orc_trapezoid* out) {
+  memset(out, 0, sizeof(*out));
+  double P = 1.0 / f;
+  double q0 = (double)m / (double)nb;
+  double D0 = q0 * P;
+  double win = 2.0 * D0;
+  double* buf = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1) * 3);
+  double *dtv = buf, *yv = buf + n, *wv = buf + 2 * n;
+  int64_t nf = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    double x = (t[i] - t0_bls) / P;
+    double cyc = floor(x + 0.5);
+    double dt = (x - cyc) * P;
+    if (fabs(dt) <= win) { dtv[nf] = dt; yv[nf] = y[i]; wv[nf] = 1.0 / (dy[i] * dy[i]); ++nf; }
+  }
+  out->n_fit = (int32_t)nf;
+  out->t0 = t0_bls; out->q = q0; out->q_in = 0.25;
+  if (nf < 5) { out->status = 2; free(buf); return; }
+  double A = 0.0, E = 0.0;
+  for (int64_t i = 0; i < nf; ++i) { A += wv[i]; E += wv[i] * yv[i]; }
+  double ybar = E / A, G = 0.0;
+  for (int64_t i = 0; i < nf; ++i) { yv[i] = yv[i] - ybar; G += wv[i] * yv[i] * yv[i]; }
+  orc_fit_data fd = {nf, dtv, yv, wv, A, ybar, G, P};
+  double th[3] = {0.0, q0, 0.25};
+  double h[3] = {0.25 * D0, 0.25 * q0, 0.125};
+  const double lo[3] = {-D0, 0.0, 0.0}, hi[3] = {D0, 1.0, 0.5};
+  double dl, z;
+  double best = orc_trap_chi2(&fd, th[0], th[1], th[2], &dl, &z);
+  int n_eval = 1;
+  out->chi2_init = best;
+  for (int level = 0; level < 24 && n_eval < 600; ++level) {
+    int moved = 1;
+    while (moved && n_eval < 600) {
+      moved = 0;
+      for (int d = 0; d < 3; ++d) {
+        for (int sg = 0; sg < 2; ++sg) {
+          double c[3] = {th[0], th[1], th[2]};
+          double v = sg == 0 ? th[d] + h[d] : th[d] - h[d];
+          if (v < lo[d]) v = lo[d];
+          if (v > hi[d]) v = hi[d];
+          if (v == th[d]) continue;
+          c[d] = v;
+          double dl2, z2;
+          double chi = orc_trap_chi2(&fd, c[0], c[1], c[2], &dl2, &z2);
+          ++n_eval;
+          if (chi < best) { best = chi; th[d] = v; dl = dl2; z = z2; moved = 1; }
+        }
+      }
+    }
+    h[0] *= 0.5; h[1] *= 0.5; h[2] *= 0.5;
+  }
+  out->t0 = t0_bls + th[0]; out->q = th[1]; out->q_in = th[2];
+  out->depth = dl; out->z = z; out->chi2 = best; out->n_eval = n_eval; out->status = 0;
+  free(buf);
+}
+int orc_sizeof_trapezoid(void) { return (int)sizeof(orc_trapezoid); }
