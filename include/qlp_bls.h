@@ -121,6 +121,25 @@ typedef struct {
   double duration;     /* D = (m / nb) * period, days                                              */
 } qlp_bls_transit_stats;
 
+/* Trapezoid fit of one peak, written by qlp_bls_trapezoid_fit() (device memory, [S * top_k], same
+ * order as the peak table).  DESIGN.md O8: model y ~ z - depth * sh(|dt - (t0 - t0_bls)|) with sh the unit trapezoid
+ * of total duration q P and ingress q_in q P; P = 1/freq stays fixed; the data are the points within two BLS
+ * durations of the BLS mid-transit times.  status: 0 fitted, 1 no peak (all fields of the start point), 2 fewer than
+ * 5 points in the window (not fitted: t0, q of the BLS, q_in = 0.25). */
+typedef struct {
+  double t0;          /* transit epoch (same zero point as t)                                       */
+  double depth;       /* > 0 for a dip of y (sign convention of qlp_bls_peak.depth)                 */
+  double q;           /* duration / period, in [0, 1]                                               */
+  double q_in;        /* ingress duration / duration, in [0, 0.5]                                   */
+  double z;           /* out-of-transit level, unit of y                                            */
+  double chi2;        /* sum dy^-2 (y - model)^2 over the fitted points                             */
+  double chi2_init;   /* the same at the start point (t0_bls, q_bls, 0.25)                          */
+  int32_t n_fit;      /* points in the window                                                       */
+  int32_t n_eval;     /* chi2 evaluations spent (no sweep of six starts after 600)                  */
+  int32_t status;
+  int32_t pad_;
+} qlp_bls_trapezoid;
+
 /* Fill *cfg with the paper's defaults, device 0, top_k 3. */
 void qlp_bls_default_config(qlp_bls_config* cfg /*host*/);
 
@@ -164,6 +183,15 @@ int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const
  *   out: stats dev [S * top_k]. */
 int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
                        const double* dy, const qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, void* cuda_stream);
+
+/* Trapezoid fit of every peak (O8): epoch, depth, q, q_in and level by
+ * least squares at the fixed BLS period, from the BLS values, on the points within two durations of mid-transit.
+ *   in : the batch (row_ptr, t, y, dy) and the peak table written by qlp_bls_snr, all dev.
+ *   out: fits dev [S * top_k].
+ * Synchronises the stream once (the workspace is sized from the number of points inside the fit windows).
+ * Returns EUNSUPPORTED if one window holds 2^31 points or more. */
+int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
+                          const double* dy, const qlp_bls_peak* peaks, qlp_bls_trapezoid* fits, void* cuda_stream);
 
 /* Whole path with HOST buffers (pageable or pinned): copies the batch to the device in sub-batches (the copy of
  * the next one overlaps the search of the current one), runs grid -> spectrum -> snr (-> peak_stats), copies the

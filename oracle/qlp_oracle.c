@@ -494,7 +494,7 @@ int orc_sizeof_peak_stats(void) { return (int)sizeof(orc_peak_stats); }
  *   search   : compass search over (c, q, q_in) from (0, q0, 0.25) with steps (D0/4, q0/4, 0.125), bounds
  *              c in [-D0, D0], q in [0, 1], q_in in [0, 0.5]: sweep the six moves (+,- per coordinate, in
  *              that order), accept a move iff chi2 strictly decreases; when a sweep accepts nothing halve the
- *              steps; 24 halvings; at most 600 evaluations.
+ *              steps; 24 halvings; no sweep starts once 600 evaluations are spent (so at most 605).
  * FP64; the sums run over the selected points in time order. */
 typedef struct {
   double t0, depth, q, q_in, z, chi2, chi2_init;

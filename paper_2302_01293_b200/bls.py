@@ -37,7 +37,11 @@ PEAK_DTYPE = np.dtype([("k", "i8"), ("freq", "f8"), ("period", "f8"), ("t0", "f8
 STATS_DTYPE = np.dtype([("n_in", "i4"), ("n_before", "i4"), ("n_after", "i4"), ("n_transits", "i4"),
                         ("oot_level", "f8"), ("duration", "f8")], align=True)
 
-EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
+TRAP_DTYPE = np.dtype([("t0", "f8"), ("depth", "f8"), ("q", "f8"), ("q_in", "f8"), ("z", "f8"), ("chi2", "f8"),
+                       ("chi2_init", "f8"), ("n_fit", "i4"), ("n_eval", "i4"), ("status", "i4"), ("pad_", "i4")],
+                      align=True)
+
+EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
            "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
@@ -61,6 +65,7 @@ def load_library():
         L.qlp_bls_spectrum.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_snr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_peak_stats.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
+        L.qlp_bls_trapezoid_fit.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_search_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
         L.qlp_bls_destroy.argtypes = [vp]
         L.qlp_bls_strerror.argtypes = [C.c_int]
@@ -211,6 +216,17 @@ class QlpBls:
                                            _ptr(stats), self._stream()), "qlp_bls_peak_stats")
         return stats
 
+    # -- O8
+    def trapezoid_fit(self, row_ptr, t, y, dy, peaks):
+        """qlp_bls_trapezoid_fit -> fits uint8[S*top_k, 72] tensor (see fits_to_numpy).  Synchronises once."""
+        torch = self.torch
+        S = int(row_ptr.numel()) - 1
+        fits = torch.zeros((max(S * self.top_k, 1), TRAP_DTYPE.itemsize), dtype=torch.uint8,
+                           device=self.device)[:S * self.top_k]
+        _check(self.lib.qlp_bls_trapezoid_fit(self._h, S, _ptr(row_ptr), _ptr(t), _ptr(y), _ptr(dy), _ptr(peaks),
+                                              _ptr(fits), self._stream()), "qlp_bls_trapezoid_fit")
+        return fits
+
     # -- whole path from host (numpy / pinned torch CPU) buffers
     def search_host(self, row_ptr, t, y, dy, rho, want_grid: bool = False, want_stats: bool = False):
         """qlp_bls_search_host on numpy arrays -> (peaks structured [S, top_k], grid or None, total_freq)
@@ -270,6 +286,11 @@ def peaks_to_numpy(peaks_tensor, top_k: int) -> np.ndarray:
 
 def stats_to_numpy(stats_tensor, top_k: int) -> np.ndarray:
     a = np.frombuffer(stats_tensor.cpu().numpy().tobytes(), dtype=STATS_DTYPE).copy()
+    return a.reshape(-1, top_k)
+
+
+def fits_to_numpy(fits_tensor, top_k: int) -> np.ndarray:
+    a = np.frombuffer(fits_tensor.cpu().numpy().tobytes(), dtype=TRAP_DTYPE).copy()
     return a.reshape(-1, top_k)
 
 

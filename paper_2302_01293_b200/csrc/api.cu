@@ -11,6 +11,7 @@
 #include "prep.cuh"
 #include "snr_kernel.cuh"
 #include "stats.cuh"
+#include "fit.cuh"
 
 using namespace qlp;
 
@@ -43,7 +44,7 @@ struct qlp_bls_ctx {
   int32_t force_path = 0;
   int64_t launches = 0;
   // workspace
-  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev;
+  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work;
   // host-API staging
   DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats;
   static const int kSide = 3;           // side streams for the independent tile-class launches
@@ -173,7 +174,7 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   if (!ctx) return QLP_BLS_OK;
   cudaSetDevice(ctx->device);
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
-                    &ctx->totals_dev, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
+                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
                     &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats};
   for (DevBuf* b : bufs) b->release();
@@ -430,6 +431,41 @@ extern "C" int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64
   CUDA_TRY(cudaSetDevice(ctx->device));
   peak_stats_kernel<<<(unsigned)(n_stars * ctx->prm.top_k), 256, 0, (cudaStream_t)cuda_stream>>>(
       n_stars, ctx->prm.top_k, row_ptr, t, y, dy, peaks, stats);
+  return launch_ok(ctx);
+}
+
+// ---- O8: trapezoid fit of every peak --------------------------------------------------------------------
+extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                     const double* y, const double* dy, const qlp_bls_peak* peaks,
+                                     qlp_bls_trapezoid* fits, void* cuda_stream) {
+  if (!ctx || n_stars < 0) return QLP_BLS_EINVAL;
+  if (n_stars == 0) return QLP_BLS_OK;
+  if (!row_ptr || !t || !y || !dy || !peaks || !fits) return QLP_BLS_EINVAL;
+  const int64_t n_items = n_stars * ctx->prm.top_k;
+  if (n_items > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  int rc = ctx->fit_cnt.ensure((size_t)n_items * sizeof(int64_t));
+  if (rc == 0) rc = ctx->fit_off.ensure((size_t)(n_items + 2) * sizeof(int64_t));
+  if (rc != 0) return rc;
+  int64_t* cnt = (int64_t*)ctx->fit_cnt.p;
+  int64_t* off = (int64_t*)ctx->fit_off.p;
+  const unsigned n_cta = (unsigned)((n_items + kFitWarps - 1) / kFitWarps);
+  fit_count_kernel<<<n_cta, kFitWarps * 32, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, peaks, cnt);
+  rc = launch_ok(ctx);
+  if (rc != 0) return rc;
+  fit_scan_kernel<<<1, 1024, 0, st>>>(n_items, cnt, off, off + n_items + 1);
+  rc = launch_ok(ctx);
+  if (rc != 0) return rc;
+  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 2, off + n_items, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  const int64_t total = ctx->totals_host[2];
+  if (total < 0) return QLP_BLS_ECUDA;
+  // a single window never holds more points than its star, and a star is capped at QLP_BLS_MAX_POINTS < 2^31
+  rc = ctx->fit_work.ensure((size_t)(total > 0 ? total : 1) * 3 * sizeof(double));
+  if (rc != 0) return rc;
+  fit_kernel<<<n_cta, kFitWarps * 32, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks, off,
+                                                (double*)ctx->fit_work.p, fits);
   return launch_ok(ctx);
 }
 
