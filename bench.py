@@ -273,6 +273,18 @@ def run_gpu(args):
     ph = ctx.fold_phase_clocks()
     ctx.fold_timing(False)
 
+    # the row after the search, measured on its own: it is not part of `value`
+    ctx.trapezoid_fit(row_ptr, t, y, dy, peaks)
+    torch.cuda.synchronize()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for _ in range(args.steps):
+        fits = ctx.trapezoid_fit(row_ptr, t, y, dy, peaks)
+    f1.record()
+    torch.cuda.synchronize()
+    fit_ms = f0.elapsed_time(f1) / args.steps
+    fit_np = bls.fits_to_numpy(fits, ctx.top_k)
+
     # end to end through the host-buffer API: pinned host inputs, H2D and D2H inside the timed region
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     h = [pin(batch.row_ptr), pin(batch.t), pin(batch.y), pin(batch.dy), pin(batch.rho)]
@@ -311,6 +323,10 @@ def run_gpu(args):
         "e2e": {"value": evals_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "stars_per_s": stars_all * args.steps / (e2e_ms * 1e-3)},
         "gpu_launches": int(launches),
+        # rank 0's shard, outside the timed region of `value`: count + scan + fit kernels of qlp_bls_trapezoid_fit
+        "trapezoid_fit": {"ms_per_call": fit_ms, "fits": int(fit_np.size), "fits_per_s": fit_np.size / (fit_ms * 1e-3),
+                          "mean_points_per_fit": float(fit_np["n_fit"].mean()),
+                          "mean_chi2_evaluations": float(fit_np["n_eval"].mean())},
         "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
                      "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",
                      "frac": achieved / peak if peak > 0 else None,

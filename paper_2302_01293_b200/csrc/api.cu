@@ -157,6 +157,8 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
                                  smem_for_cols(CT_)) == cudaSuccess &&                                               \
             cudaFuncSetAttribute(foldscan_kernel<16, CT_, 0u>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
                                  smem_for_cols(CT_)) == cudaSuccess
+  attr_ok = attr_ok && cudaFuncSetAttribute(fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            kFitSmemBytes) == cudaSuccess;
   QLP_ATTR(128); QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
   if (!attr_ok ||
       cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
@@ -464,7 +466,7 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
   // a single window never holds more points than its star, and a star is capped at QLP_BLS_MAX_POINTS < 2^31
   rc = ctx->fit_work.ensure((size_t)(total > 0 ? total : 1) * 3 * sizeof(double));
   if (rc != 0) return rc;
-  fit_kernel<<<n_cta, kFitWarps * 32, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks, off,
+  fit_kernel<<<(unsigned)n_items, kFitThreads, kFitSmemBytes, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks, off,
                                                 (double*)ctx->fit_work.p, fits);
   return launch_ok(ctx);
 }
