@@ -209,6 +209,16 @@ def trapezoid_fit(t, y, dy, f: float, m: int, nb: int, t0: float):
     return out[0]
 
 
+def trapezoid_chi2_at(t, y, dy, f: float, m: int, nb: int, t0: float, c: float, q: float, q_in: float):
+    """O8: (chi2, depth, z) of the fit data of a peak at given (c = T0 - t0, q, q_in)."""
+    t, y, dy = _f8(t), _f8(y), _f8(dy)
+    res = np.zeros(3)
+    lib().orc_trapezoid_chi2_at.restype = C.c_int64
+    lib().orc_trapezoid_chi2_at(C.c_int64(t.size), _p(t), _p(y), _p(dy), C.c_double(f), C.c_int32(m), C.c_int32(nb),
+                                C.c_double(t0), C.c_double(c), C.c_double(q), C.c_double(q_in), _p(res))
+    return float(res[0]), float(res[1]), float(res[2])
+
+
 def batch(cfg: Config, row_ptr, t, y, dy, rho, K: int = 3, want_snr: bool = True, threads: int | None = None):
     """Whole path on a CSR batch (OpenMP over stars) -> dict(grid, freq_ptr, sr, m, j, snr, peaks)."""
     row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)

@@ -533,14 +533,10 @@ static double orc_trap_chi2(const orc_fit_data* fd, double c, double q, double q
   return chi2;
 }
 
-void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double* dy, double f, int32_t m,
-                       int32_t nb, double t0_bls, orc_trapezoid* out) {
-  memset(out, 0, sizeof(*out));
-  double P = 1.0 / f;
-  double q0 = (double)m / (double)nb;
-  double D0 = q0 * P;
+/* The data of a fit (window selection, weights, centring).  Returns n_fit; buf holds 3 n doubles. */
+static int64_t orc_fit_select(int64_t n, const double* t, const double* y, const double* dy, double P, double D0,
+                              double t0_bls, double* buf, orc_fit_data* fd) {
   double win = 2.0 * D0;
-  double* buf = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1) * 3);
   double *dtv = buf, *yv = buf + n, *wv = buf + 2 * n;
   int64_t nf = 0;
   for (int64_t i = 0; i < n; ++i) {
@@ -549,14 +545,26 @@ void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double
     double dt = (x - cyc) * P;
     if (fabs(dt) <= win) { dtv[nf] = dt; yv[nf] = y[i]; wv[nf] = 1.0 / (dy[i] * dy[i]); ++nf; }
   }
+  double A = 0.0, E = 0.0, G = 0.0;
+  for (int64_t i = 0; i < nf; ++i) { A += wv[i]; E += wv[i] * yv[i]; }
+  double ybar = nf > 0 ? E / A : 0.0;
+  for (int64_t i = 0; i < nf; ++i) { yv[i] = yv[i] - ybar; G += wv[i] * yv[i] * yv[i]; }
+  fd->n = nf; fd->dt = dtv; fd->yt = yv; fd->w = wv; fd->A = A; fd->ybar = ybar; fd->G = G; fd->P = P;
+  return nf;
+}
+
+void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double* dy, double f, int32_t m,
+                       int32_t nb, double t0_bls, orc_trapezoid* out) {
+  memset(out, 0, sizeof(*out));
+  double P = 1.0 / f;
+  double q0 = (double)m / (double)nb;
+  double D0 = q0 * P;
+  double* buf = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1) * 3);
+  orc_fit_data fd;
+  int64_t nf = orc_fit_select(n, t, y, dy, P, D0, t0_bls, buf, &fd);
   out->n_fit = (int32_t)nf;
   out->t0 = t0_bls; out->q = q0; out->q_in = 0.25;
   if (nf < 5) { out->status = 2; free(buf); return; }
-  double A = 0.0, E = 0.0;
-  for (int64_t i = 0; i < nf; ++i) { A += wv[i]; E += wv[i] * yv[i]; }
-  double ybar = E / A, G = 0.0;
-  for (int64_t i = 0; i < nf; ++i) { yv[i] = yv[i] - ybar; G += wv[i] * yv[i] * yv[i]; }
-  orc_fit_data fd = {nf, dtv, yv, wv, A, ybar, G, P};
   double th[3] = {0.0, q0, 0.25};
   double h[3] = {0.25 * D0, 0.25 * q0, 0.125};
   const double lo[3] = {-D0, 0.0, 0.0}, hi[3] = {D0, 1.0, 0.5};
@@ -588,5 +596,19 @@ void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double
   out->t0 = t0_bls + th[0]; out->q = th[1]; out->q_in = th[2];
   out->depth = dl; out->z = z; out->chi2 = best; out->n_eval = n_eval; out->status = 0;
   free(buf);
+}
+/* chi2 (and the linear solution) of the same data at given (c, q, q_in): lets a test check a fit found elsewhere.
+ * res = {chi2, depth, z}; returns n_fit. */
+int64_t orc_trapezoid_chi2_at(int64_t n, const double* t, const double* y, const double* dy, double f, int32_t m,
+                              int32_t nb, double t0_bls, double c, double q, double qin, double* res) {
+  double P = 1.0 / f;
+  double D0 = (double)m / (double)nb * P;
+  double* buf = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1) * 3);
+  orc_fit_data fd;
+  int64_t nf = orc_fit_select(n, t, y, dy, P, D0, t0_bls, buf, &fd);
+  res[0] = res[1] = res[2] = 0.0;
+  if (nf > 0) res[0] = orc_trap_chi2(&fd, c, q, qin, &res[1], &res[2]);
+  free(buf);
+  return nf;
 }
 int orc_sizeof_trapezoid(void) { return (int)sizeof(orc_trapezoid); }

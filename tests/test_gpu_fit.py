@@ -3,9 +3,11 @@
 Both sides run the same compass search in FP64 on the same points.  The window membership is an integer decision
 taken with the same unfused operations (n_fit: bit-exact).  The trial parameters are sums and halvings of the same
 numbers, so the two paths are identical unless a chi2 comparison falls inside the rounding noise of two summation
-orders (relative 1e-13); the tolerance below allows for the last few steps of a search ending differently:
-chi2 within 1e-9 relative (+ 1e-12 of chi2_init for fits that reach zero), epoch within 1e-6 of the BLS duration,
-q within 1e-6 relative, q_in within 1e-5, depth and level within 1e-6 of the depth."""
+orders (relative 1e-13), which happens on noise peaks whose chi2 is flat along some direction (measured: about one
+fit in twelve, parameters then differ by up to 4e-5 relative at equal chi2).  So the test compares what is unique --
+the minimum reached (1e-8 relative) -- checks that the GPU's parameters are valid by evaluating the ORACLE's chi2,
+depth and level at them (1e-9 / 1e-6), bounds the parameter differences (1e-3), and demands that at least 70 % of the
+fits end at the same point (1e-9) after the same number of evaluations."""
 import numpy as np
 import pytest
 
@@ -31,22 +33,32 @@ def run_search(gpu, ctx, b):
     return gpu.peaks_to_numpy(peaks, ctx.top_k), fits
 
 
-def compare(g, o, p):
+def compare(orc, star, g, o, p):
+    """g: GPU fit, o: oracle fit, p: the peak.  Returns True if both searches ended at the same point (1e-9)."""
+    t, y, dy = star
     D0 = p["m"] / p["nb"] * p["period"]
     assert g["n_fit"] == o["n_fit"] and g["status"] == o["status"]
     if o["status"] != 0:
         assert g["t0"] == o["t0"] and g["q"] == o["q"] and g["q_in"] == o["q_in"]
-        return
+        return True
+    floor = 1e-12 * o["chi2_init"]
+    # what is unique: the start value and the minimum reached
     assert abs(g["chi2_init"] - o["chi2_init"]) <= 1e-9 * o["chi2_init"]
-    assert abs(g["chi2"] - o["chi2"]) <= 1e-9 * o["chi2"] + 1e-12 * o["chi2_init"]
-    assert abs(g["t0"] - o["t0"]) <= 1e-6 * D0
-    assert abs(g["q"] - o["q"]) <= 1e-6 * o["q"]
-    assert abs(g["q_in"] - o["q_in"]) <= 1e-5
-    scale = max(abs(o["depth"]), 1e-12)
-    assert abs(g["depth"] - o["depth"]) <= 1e-6 * scale
-    assert abs(g["z"] - o["z"]) <= 1e-6 * scale + 1e-12 * abs(o["z"])
+    assert abs(g["chi2"] - o["chi2"]) <= 1e-8 * o["chi2"] + floor
+    # the GPU's parameters are valid: the oracle's chi2, depth and level AT those parameters are the GPU's
+    c2, depth, z = orc.trapezoid_chi2_at(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]),
+                                         float(g["t0"] - p["t0"]), float(g["q"]), float(g["q_in"]))
+    scale = max(abs(depth), 1e-12)
+    assert abs(g["chi2"] - c2) <= 1e-9 * c2 + floor
+    assert abs(g["depth"] - depth) <= 1e-6 * scale and abs(g["z"] - z) <= 1e-6 * scale + 1e-12 * abs(z)
     assert g["chi2"] <= g["chi2_init"] and 0.0 <= g["q"] <= 1.0 and 0.0 <= g["q_in"] <= 0.5
-    assert abs(int(g["n_eval"]) - int(o["n_eval"])) <= 12 and g["n_eval"] <= 605
+    assert abs(g["t0"] - p["t0"]) <= D0 and g["n_eval"] <= 605
+    # the parameters themselves: equal when both searches took the same path, else equally good neighbours
+    # (on a noise peak chi2 is flat to ~1e-13 along some directions and the summation order decides a move)
+    assert abs(g["t0"] - o["t0"]) <= 1e-3 * D0
+    assert abs(g["q"] - o["q"]) <= 1e-3 * o["q"] and abs(g["q_in"] - o["q_in"]) <= 2e-3
+    return bool(int(g["n_eval"]) == int(o["n_eval"]) and abs(g["t0"] - o["t0"]) <= 1e-9 * D0 and
+                abs(g["q"] - o["q"]) <= 1e-9 * o["q"] and abs(g["q_in"] - o["q_in"]) <= 1e-9)
 
 
 @pytest.mark.parametrize("config,ids", [(1, [0]), (2, list(range(8))), (5, [0, 1, 2, 3, 19, 28])])
@@ -56,7 +68,7 @@ def test_trapezoid_fit_matches_oracle(gpu, orc, config, ids):
     ctx = gpu.QlpBls(top_k=3)
     try:
         pk, fits = run_search(gpu, ctx, b)
-        checked = 0
+        checked = same_path = 0
         for s in range(b.n_stars):
             t, y, dy = b.star(s)
             for r in range(ctx.top_k):
@@ -65,9 +77,9 @@ def test_trapezoid_fit_matches_oracle(gpu, orc, config, ids):
                     assert g["status"] == 1 and g["n_fit"] == 0
                     continue
                 o = orc.trapezoid_fit(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]))
-                compare(g, o, p)
+                same_path += compare(orc, (t, y, dy), g, o, p)
                 checked += 1
-        assert checked >= b.n_stars
+        assert checked >= b.n_stars and same_path >= 0.7 * checked
         if config == 1:  # the injected transit of BASELINE.json configs[0]: the fit keeps the BLS depth within 2x
             assert fits[0][0]["status"] == 0 and 0.5 * pk[0][0]["depth"] < fits[0][0]["depth"] < 2.0 * pk[0][0]["depth"]
             assert fits[0][0]["chi2"] < fits[0][0]["chi2_init"]
@@ -100,9 +112,9 @@ def test_trapezoid_fit_recovers_an_injected_trapezoid(gpu, orc):
             assert abs(g["q"] * p["period"] - D) < 0.2 * D and abs(g["depth"] - depth) < 0.1 * depth
             assert abs(g["z"] - 1.0) < 1e-4 and 0.0 < g["q_in"] <= 0.5
             assert g["chi2"] < g["chi2_init"]
-        o = orc.trapezoid_fit(t, y, np.full(t.size, 1e-3), float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]))
-        assert g["n_fit"] == o["n_fit"]
-        assert abs(g["chi2"] - o["chi2"]) <= 1e-6 * o["chi2_init"]
+        dy = np.full(t.size, 1e-3)
+        o = orc.trapezoid_fit(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]))
+        compare(orc, (t, y, dy), g, o, p)
     finally:
         ctx.close()
 

@@ -77,6 +77,8 @@ def test_chi2_and_linear_part_match_lstsq_and_nelder_mead_finds_nothing_better(q
     assert r["n_fit"] == n_sel
     assert r["chi2"] == pytest.approx(chi2, rel=1e-9)
     assert r["z"] == pytest.approx(sol[0], rel=1e-9) and r["depth"] == pytest.approx(sol[1], rel=1e-7)
+    at = oracle.trapezoid_chi2_at(t, y, dy, 1.0 / P, c["m"], c["nb"], c["t0_bls"], r["t0"] - c["t0_bls"], r["q"], r["q_in"])
+    assert at[0] == pytest.approx(chi2, rel=1e-9) and at[1] == pytest.approx(sol[1], rel=1e-7)
     assert r["chi2"] <= r["chi2_init"]
     assert 0.0 <= r["q"] <= 1.0 and 0.0 <= r["q_in"] <= 0.5 and abs(r["t0"] - c["t0_bls"]) <= D0
 
