@@ -219,6 +219,20 @@ def trapezoid_chi2_at(t, y, dy, f: float, m: int, nb: int, t0: float, c: float, 
     return float(res[0]), float(res[1]), float(res[2])
 
 
+PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8"), ("snr_pink", "f8"),
+                       ("n_t", "i4"), ("n_transits", "i4"), ("n_bins", "i4"), ("detected", "i4")], align=True)
+
+
+def pink_noise(t, y, f: float, t0: float, depth: float, q: float, q_in: float, z: float, snr: float):
+    """O9: sigma_w, sigma_r on the duration timescale, S/N_pink (Eq. 2), detection flag."""
+    t, y = _f8(t), _f8(y)
+    out = np.zeros(1, dtype=PINK_DTYPE)
+    assert lib().orc_sizeof_pink() == PINK_DTYPE.itemsize
+    lib().orc_pink_noise(C.c_int64(t.size), _p(t), _p(y), C.c_double(f), C.c_double(t0), C.c_double(depth),
+                         C.c_double(q), C.c_double(q_in), C.c_double(z), C.c_double(snr), _p(out))
+    return out[0]
+
+
 def batch(cfg: Config, row_ptr, t, y, dy, rho, K: int = 3, want_snr: bool = True, threads: int | None = None):
     """Whole path on a CSR batch (OpenMP over stars) -> dict(grid, freq_ptr, sr, m, j, snr, peaks)."""
     row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)

@@ -20,6 +20,7 @@
  *   O3 bin index                O4 box scan -> SR(f), best (m, j)
  *   O5 S/N spectrum (footnote 3 at :65)   O6 peaks
  *   O7 per-peak statistics                  O8 trapezoid fit
+ *   O9 sigma_w, sigma_r, S/N_pink, detection criteria
  */
 #include <math.h>
 #include <stdint.h>
@@ -612,3 +613,85 @@ int64_t orc_trapezoid_chi2_at(int64_t n, const double* t, const double* y, const
   return nf;
 }
 int orc_sizeof_trapezoid(void) { return (int)sizeof(orc_trapezoid); }
+
+/* ---------------------------------------------------------------- O9 */
+/* Noise estimates, signal-to-pink-noise and the detection criteria, PAPER.md:45-51, :55:
+ *   "we subtract the trapezoid model from the light curve and estimate the white noise (sigma_w) and red noise
+ *    (sigma_r) on the timescale of the transit duration" ... Eq. 2:
+ *        S/N_pink = delta / sqrt(sigma_w^2 / n_t + sigma_r^2 / N_t),
+ *    n_t the number of points in transit, N_t the number of transits ... "replacing delta with the integral over
+ *    the full trapezoid model" ... "detection criteria of at least two transits, S/N_pink > 9, and ... S/N > 9".
+ * The VARTOOLS noise recipe is not in the paper; readings (O9, after Pont et al. 2006):
+ *   residual r_i = y_i - (z - delta sh_i) over ALL points of the star, sh as in O8 with the fitted T0, q, q_in;
+ *   sigma_w^2 = mean (r - mean r)^2 (unweighted);
+ *   time bins of one transit duration D = q P counted from the first point, b_i = floor((t_i - t_first)/D);
+ *   m_b, n_b = mean and count of every non-empty bin;  sigma_bin^2 = mean_b (m_b - mean_b m)^2;
+ *   sigma_r^2 = max(0, sigma_bin^2 - sigma_w^2 mean_b(1/n_b))   (the white part of the binned scatter removed);
+ *   n_t, N_t as in O7 (|dt| <= D/2; a transit counts if it owns an in-transit point) with the fitted T0 and D;
+ *   delta_eff = delta (1 - q_in)   (the integral of the unit trapezoid over the duration, divided by D);
+ *   S/N_pink = delta_eff / sqrt(sigma_w^2/n_t + sigma_r^2/N_t), 0 if n_t = 0 or the denominator is 0;
+ *   detected = N_t >= 2 and S/N_pink > 9 and S/N > 9. */
+typedef struct {
+  double sigma_w, sigma_r, depth_eff, snr_pink;
+  int32_t n_t, n_transits, n_bins, detected;
+} orc_pink;
+
+void orc_pink_noise(int64_t n, const double* t, const double* y, double f, double T0, double delta, double q,
+                    double qin, double z, double snr, orc_pink* out) {
+  memset(out, 0, sizeof(*out));
+  if (n <= 0) return;
+  double P = 1.0 / f;
+  double D = q * P, half = 0.5 * D, ing = qin * D;
+  double* r = (double*)malloc(sizeof(double) * (size_t)n);
+  int32_t n_t = 0, n_tr = 0;
+  int have_prev = 0;
+  double prev_cyc = 0.0, sum = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    double x = (t[i] - T0) / P;
+    double cyc = floor(x + 0.5);
+    double dt = (x - cyc) * P;
+    double u = fabs(dt);
+    r[i] = y[i] - (z - delta * orc_trap_shape(u, half, ing));
+    sum += r[i];
+    if (u <= half) {
+      ++n_t;
+      if (!have_prev || cyc != prev_cyc) ++n_tr;
+      have_prev = 1; prev_cyc = cyc;
+    }
+  }
+  double rbar = sum / (double)n, ss = 0.0;
+  for (int64_t i = 0; i < n; ++i) ss += (r[i] - rbar) * (r[i] - rbar);
+  double var_w = ss / (double)n;
+  /* bins of one duration; t increases, so a bin is a run of consecutive points */
+  double var_bin = 0.0, mean_inv = 0.0;
+  int32_t nbins = 0;
+  if (D > 0.0) {
+    double* mb = (double*)malloc(sizeof(double) * (size_t)n);
+    double cur = floor((t[0] - t[0]) / D), acc = 0.0, inv = 0.0;
+    int64_t cnt = 0;
+    for (int64_t i = 0; i < n; ++i) {
+      double b = floor((t[i] - t[0]) / D);
+      if (b != cur) { mb[nbins++] = acc / (double)cnt; inv += 1.0 / (double)cnt; cur = b; acc = 0.0; cnt = 0; }
+      acc += r[i]; ++cnt;
+    }
+    mb[nbins++] = acc / (double)cnt; inv += 1.0 / (double)cnt;
+    double msum = 0.0;
+    for (int32_t b = 0; b < nbins; ++b) msum += mb[b];
+    double mbar = msum / (double)nbins, s2 = 0.0;
+    for (int32_t b = 0; b < nbins; ++b) s2 += (mb[b] - mbar) * (mb[b] - mbar);
+    var_bin = s2 / (double)nbins;
+    mean_inv = inv / (double)nbins;
+    free(mb);
+  }
+  double var_r = var_bin - var_w * mean_inv;
+  if (var_r < 0.0) var_r = 0.0;
+  out->sigma_w = sqrt(var_w); out->sigma_r = sqrt(var_r);
+  out->depth_eff = delta * (1.0 - qin);
+  out->n_t = n_t; out->n_transits = n_tr; out->n_bins = nbins;
+  double den = 0.0;
+  if (n_t > 0 && n_tr > 0) den = var_w / (double)n_t + var_r / (double)n_tr;
+  out->snr_pink = den > 0.0 ? out->depth_eff / sqrt(den) : 0.0;
+  out->detected = (n_tr >= 2 && out->snr_pink > 9.0 && snr > 9.0) ? 1 : 0;
+  free(r);
+}
+int orc_sizeof_pink(void) { return (int)sizeof(orc_pink); }
