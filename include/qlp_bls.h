@@ -140,6 +140,22 @@ typedef struct {
   int32_t pad_;
 } qlp_bls_trapezoid;
 
+/* Noise estimates, signal-to-pink-noise and detection flag of one peak (PAPER.md:45-51 with Eq. 2, :55), written by
+ * qlp_bls_pink_noise() (device memory, [S * top_k], same order as the peak table).  DESIGN.md O9: residuals of all
+ * points of the star against the fitted trapezoid; sigma_w = their rms about the mean; sigma_r^2 = variance of the
+ * means over time bins of one transit duration minus sigma_w^2 mean(1/n_b), floored at 0; S/N_pink = depth_eff /
+ * sqrt(sigma_w^2 / n_t + sigma_r^2 / n_transits).  Peaks without a fit (fit status != 0) give all zeros. */
+typedef struct {
+  double sigma_w;      /* white noise, unit of y                                                     */
+  double sigma_r;      /* red noise on the timescale of the fitted duration                          */
+  double depth_eff;    /* depth (1 - q_in): the trapezoid integral over the duration   */
+  double snr_pink;     /* PAPER.md Eq. 2 with depth_eff                                              */
+  int32_t n_t;         /* points in transit (fitted epoch and duration)                              */
+  int32_t n_transits;  /* transits with data within 0.5 durations of mid-transit                     */
+  int32_t n_bins;      /* non-empty duration-long time bins                                          */
+  int32_t detected;    /* 1 iff n_transits >= 2, snr_pink > 9 and the peak's S/N > 9    */
+} qlp_bls_pink;
+
 /* Fill *cfg with the paper's defaults, device 0, top_k 3. */
 void qlp_bls_default_config(qlp_bls_config* cfg /*host*/);
 
@@ -192,6 +208,13 @@ int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr
  * Returns EUNSUPPORTED if one window holds 2^31 points or more. */
 int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
                           const double* dy, const qlp_bls_peak* peaks, qlp_bls_trapezoid* fits, void* cuda_stream);
+
+/* Noise estimates, S/N_pink and the detection criteria of every peak (O9; SURVEY.md
+ * 8(f) f3).
+ *   in : the batch (row_ptr, t, y), the peak table of qlp_bls_snr and the fits of qlp_bls_trapezoid_fit, all dev.
+ *   out: pink dev [S * top_k].  Asynchronous on the stream. */
+int qlp_bls_pink_noise(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
+                       const qlp_bls_peak* peaks, const qlp_bls_trapezoid* fits, qlp_bls_pink* pink, void* cuda_stream);
 
 /* Whole path with HOST buffers (pageable or pinned): copies the batch to the device in sub-batches (the copy of
  * the next one overlaps the search of the current one), runs grid -> spectrum -> snr (-> peak_stats), copies the

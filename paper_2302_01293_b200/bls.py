@@ -41,7 +41,10 @@ TRAP_DTYPE = np.dtype([("t0", "f8"), ("depth", "f8"), ("q", "f8"), ("q_in", "f8"
                        ("chi2_init", "f8"), ("n_fit", "i4"), ("n_eval", "i4"), ("status", "i4"), ("pad_", "i4")],
                       align=True)
 
-EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
+PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8"), ("snr_pink", "f8"),
+                       ("n_t", "i4"), ("n_transits", "i4"), ("n_bins", "i4"), ("detected", "i4")], align=True)
+
+EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
            "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
@@ -66,6 +69,7 @@ def load_library():
         L.qlp_bls_snr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_peak_stats.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_trapezoid_fit.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
+        L.qlp_bls_pink_noise.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_search_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
         L.qlp_bls_destroy.argtypes = [vp]
         L.qlp_bls_strerror.argtypes = [C.c_int]
@@ -227,6 +231,17 @@ class QlpBls:
                                               _ptr(fits), self._stream()), "qlp_bls_trapezoid_fit")
         return fits
 
+    # -- O9
+    def pink_noise(self, row_ptr, t, y, peaks, fits):
+        """qlp_bls_pink_noise -> pink uint8[S*top_k, 48] tensor (see pink_to_numpy)."""
+        torch = self.torch
+        S = int(row_ptr.numel()) - 1
+        pink = torch.zeros((max(S * self.top_k, 1), PINK_DTYPE.itemsize), dtype=torch.uint8,
+                           device=self.device)[:S * self.top_k]
+        _check(self.lib.qlp_bls_pink_noise(self._h, S, _ptr(row_ptr), _ptr(t), _ptr(y), _ptr(peaks), _ptr(fits),
+                                           _ptr(pink), self._stream()), "qlp_bls_pink_noise")
+        return pink
+
     # -- whole path from host (numpy / pinned torch CPU) buffers
     def search_host(self, row_ptr, t, y, dy, rho, want_grid: bool = False, want_stats: bool = False):
         """qlp_bls_search_host on numpy arrays -> (peaks structured [S, top_k], grid or None, total_freq)
@@ -291,6 +306,11 @@ def stats_to_numpy(stats_tensor, top_k: int) -> np.ndarray:
 
 def fits_to_numpy(fits_tensor, top_k: int) -> np.ndarray:
     a = np.frombuffer(fits_tensor.cpu().numpy().tobytes(), dtype=TRAP_DTYPE).copy()
+    return a.reshape(-1, top_k)
+
+
+def pink_to_numpy(pink_tensor, top_k: int) -> np.ndarray:
+    a = np.frombuffer(pink_tensor.cpu().numpy().tobytes(), dtype=PINK_DTYPE).copy()
     return a.reshape(-1, top_k)
 
 

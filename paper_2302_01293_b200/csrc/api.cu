@@ -12,6 +12,7 @@
 #include "snr_kernel.cuh"
 #include "stats.cuh"
 #include "fit.cuh"
+#include "pink.cuh"
 
 using namespace qlp;
 
@@ -468,6 +469,20 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
   if (rc != 0) return rc;
   fit_kernel<<<(unsigned)n_items, kFitThreads, kFitSmemBytes, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks, off,
                                                 (double*)ctx->fit_work.p, fits);
+  return launch_ok(ctx);
+}
+
+// ---- O9: noise estimates, S/N_pink, detection criteria ------------------------------------------------
+extern "C" int qlp_bls_pink_noise(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                  const double* y, const qlp_bls_peak* peaks, const qlp_bls_trapezoid* fits,
+                                  qlp_bls_pink* pink, void* cuda_stream) {
+  if (!ctx || n_stars < 0) return QLP_BLS_EINVAL;
+  if (n_stars == 0) return QLP_BLS_OK;
+  if (!row_ptr || !t || !y || !peaks || !fits || !pink) return QLP_BLS_EINVAL;
+  if (n_stars * ctx->prm.top_k > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  pink_kernel<<<(unsigned)(n_stars * ctx->prm.top_k), kPinkThreads, 0, (cudaStream_t)cuda_stream>>>(
+      n_stars, ctx->prm.top_k, row_ptr, t, y, peaks, fits, pink);
   return launch_ok(ctx);
 }
 

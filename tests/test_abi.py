@@ -36,7 +36,7 @@ def test_struct_layouts(lib):
     from paper_2302_01293_b200 import bls
     assert bls.GRID_DTYPE.itemsize == 72
     assert bls.PEAK_DTYPE.itemsize == 64
-    assert bls.STATS_DTYPE.itemsize == 32 and bls.TRAP_DTYPE.itemsize == 72
+    assert bls.STATS_DTYPE.itemsize == 32 and bls.TRAP_DTYPE.itemsize == 72 and bls.PINK_DTYPE.itemsize == 48
     cfg = bls.default_config()
     assert cfg.struct_bytes == C.sizeof(bls.Config) == 72
     # the paper's parameters: PAPER.md:35 (samples_per_peak=2, dlogq=0.1, noverlap=3), :19, :23, :7

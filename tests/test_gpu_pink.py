@@ -1,0 +1,113 @@
+"""O9 parity on the GPU: sigma_w, sigma_r, S/N_pink and the detection flag against the oracle,
+through the C ABI.  Both sides get the SAME fit (the GPU's), so this checks the noise kernel alone.  Counts (points in
+transit, transits, non-empty bins) are integer decisions taken with the same unfused FP64 operations: bit-exact.
+The variances are FP64 sums in another order (single pass, shifted): sigma_w within 1e-9 relative, sigma_r within
+1e-6 of sigma_w (it is the square root of a difference floored at zero), S/N_pink within 1e-6 relative."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2302_01293_b200 import build, bls
+    build.build()
+    return bls
+
+
+def run(gpu, ctx, b):
+    dev = gpu.upload(b)
+    grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+    _, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best, want_snr=False)
+    fits = ctx.trapezoid_fit(dev[0], dev[1], dev[2], dev[3], peaks)
+    pink = ctx.pink_noise(dev[0], dev[1], dev[2], peaks, fits)
+    return (gpu.peaks_to_numpy(peaks, ctx.top_k), gpu.fits_to_numpy(fits, ctx.top_k),
+            gpu.pink_to_numpy(pink, ctx.top_k))
+
+
+def compare(orc, star, p, ft, g):
+    t, y, _ = star
+    o = orc.pink_noise(t, y, float(p["freq"]), float(ft["t0"]), float(ft["depth"]), float(ft["q"]), float(ft["q_in"]),
+                       float(ft["z"]), float(p["snr"]))
+    for k in ("n_t", "n_transits", "n_bins"):
+        assert g[k] == o[k], (k, g[k], o[k])
+    assert abs(g["sigma_w"] - o["sigma_w"]) <= 1e-9 * o["sigma_w"]
+    assert abs(g["sigma_r"] - o["sigma_r"]) <= 1e-6 * o["sigma_w"]
+    assert g["depth_eff"] == o["depth_eff"]
+    assert abs(g["snr_pink"] - o["snr_pink"]) <= 1e-6 * abs(o["snr_pink"]) + 1e-12
+    if abs(o["snr_pink"] - 9.0) > 1e-3:
+        assert g["detected"] == o["detected"]
+    return o
+
+
+@pytest.mark.parametrize("config,ids", [(1, [0]), (2, list(range(8))), (5, [0, 1, 2, 3, 19, 28])])
+def test_pink_noise_matches_oracle(gpu, orc, config, ids):
+    from paper_2302_01293_b200 import synth
+    b = synth.make_batch(config, star_ids=np.array(ids))
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        pk, fits, pink = run(gpu, ctx, b)
+        checked = 0
+        for s in range(b.n_stars):
+            for r in range(ctx.top_k):
+                p, ft, g = pk[s][r], fits[s][r], pink[s][r]
+                if p["k"] < 0 or ft["status"] != 0:
+                    assert g.tobytes() == bytes(48)
+                    continue
+                compare(orc, b.star(s), p, ft, g)
+                assert g["sigma_w"] > 0 and g["n_bins"] > 0
+                checked += 1
+        assert checked >= b.n_stars
+        if config == 1:  # the injected transit of BASELINE.json configs[0] passes the paper's cuts
+            assert pink[0][0]["n_transits"] >= 2 and pink[0][0]["snr_pink"] > 9.0 and pk[0][0]["snr"] > 9.0
+            assert pink[0][0]["detected"] == 1
+    finally:
+        ctx.close()
+
+
+def test_pink_noise_sees_injected_red_noise_and_rejects_a_single_transit(gpu, orc):
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(3)
+    t = synth.sector_times(0, 200.0)
+    P, T0, D, depth = 3.1, t[0] + 1.3, 0.08, 0.01
+    x = (t - T0) / P
+    dt = (x - np.floor(x + 0.5)) * P
+    box = (np.abs(dt) < 0.5 * D).astype(float)
+    white = 1e-3 * rng.standard_normal(t.size)
+    red = 1.5e-3 * np.sin(2 * np.pi * t / 0.9)
+    one = (np.abs(t - T0) < 0.5 * D).astype(float)                      # a single dip
+    stars = [(t, 1.0 - depth * box + white, np.full(t.size, 1e-3)),
+             (t, 1.0 - depth * box + white + red, np.full(t.size, 1e-3)),
+             (t, 1.0 - 3 * depth * one + white, np.full(t.size, 1e-3))]
+    b = synth.from_arrays(stars)
+    ctx = gpu.QlpBls(top_k=1)
+    try:
+        pk, fits, pink = run(gpu, ctx, b)
+        for s in range(3):
+            compare(orc, b.star(s), pk[s][0], fits[s][0], pink[s][0])
+        assert pink[0][0]["detected"] == 1 and pink[0][0]["sigma_r"] < 0.3 * pink[0][0]["sigma_w"]
+        assert pink[1][0]["sigma_r"] > 0.5e-3                           # the sinusoid shows up as red noise
+        assert pink[1][0]["snr_pink"] < pink[0][0]["snr_pink"]
+        if round(pk[2][0]["period"] / 27.0) >= 0 and pink[2][0]["n_transits"] < 2:
+            assert pink[2][0]["detected"] == 0                          # "at least two transits"
+    finally:
+        ctx.close()
+
+
+def test_pink_noise_empty_and_invalid(gpu):
+    from paper_2302_01293_b200 import synth
+    t = synth.sector_times(0, 1800.0)
+    b = synth.from_arrays([(t[:1], np.zeros(1), np.ones(1)), (t, np.zeros(t.size), np.ones(t.size))])
+    ctx = gpu.QlpBls()
+    try:
+        pk, fits, pink = run(gpu, ctx, b)
+        assert pink[0].tobytes() == bytes(48 * 3)
+        for r in range(ctx.top_k):                                      # constant series: no noise, no signal
+            assert pink[1][r]["sigma_w"] == 0.0 and pink[1][r]["snr_pink"] == 0.0 and pink[1][r]["detected"] == 0
+    finally:
+        ctx.close()
