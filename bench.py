@@ -284,6 +284,14 @@ def run_gpu(args):
     torch.cuda.synchronize()
     fit_ms = f0.elapsed_time(f1) / args.steps
     fit_np = bls.fits_to_numpy(fits, ctx.top_k)
+    ctx.pink_noise(row_ptr, t, y, peaks, fits)
+    f0.record()
+    for _ in range(args.steps):
+        pink = ctx.pink_noise(row_ptr, t, y, peaks, fits)   # O9
+    f1.record()
+    torch.cuda.synchronize()
+    pink_ms = f0.elapsed_time(f1) / args.steps
+    pink_np = bls.pink_to_numpy(pink, ctx.top_k)
 
     # end to end through the host-buffer API: pinned host inputs, H2D and D2H inside the timed region
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
@@ -327,6 +335,7 @@ def run_gpu(args):
         "trapezoid_fit": {"ms_per_call": fit_ms, "fits": int(fit_np.size), "fits_per_s": fit_np.size / (fit_ms * 1e-3),
                           "mean_points_per_fit": float(fit_np["n_fit"].mean()),
                           "mean_chi2_evaluations": float(fit_np["n_eval"].mean())},
+        "pink_noise": {"ms_per_call": pink_ms, "detected_stars": int((pink_np["detected"].max(axis=1) > 0).sum())},
         "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
                      "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",
                      "frac": achieved / peak if peak > 0 else None,
