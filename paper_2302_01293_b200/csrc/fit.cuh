@@ -12,8 +12,10 @@
 // fit_count_kernel (one warp per (star, peak)) counts the points in the window; after an exclusive scan of the
 // counts fit_kernel (one CTA per (star, peak)) compacts (dt, y, w) of its points in time order into its slice of
 // the workspace (SoA) and runs the search on them: every chi2 evaluation is one strided pass of the CTA over the
-// slice, reduced in a fixed order so that all threads hold identical values and take identical decisions.  The slice is re-read from L1/L2 (a few 10 KB per fit); the loops are unrolled so that
-// several loads are in flight per thread.
+// slice, reduced in a fixed order so that all threads hold identical values and take identical decisions.  The
+// first kFitCap points of a fit stay in shared memory (the mean window of a 200-s single-sector star holds about
+// 3,400), the rest is re-read from the slice through L1/L2; the loops are unrolled so that several loads are in
+// flight per thread.
 #pragma once
 #include "common.cuh"
 
