@@ -225,6 +225,15 @@ int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_pt
                         qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_star_grid* grid_out,
                         int64_t* total_freq, void* cuda_stream);
 
+/* qlp_bls_search_host followed, per sub-batch, by the rows after the search: trapezoid fit and noise /
+ * S/N_pink / detection flag, also copied back.  fits host [S * top_k] or NULL; pink host [S * top_k]
+ * or NULL (pink needs the fits on the device, they are computed even if fits is NULL).  Everything else as
+ * qlp_bls_search_host. */
+int qlp_bls_vet_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
+                     const double* dy, const double* rho, const double* rstar, qlp_bls_peak* peaks,
+                     qlp_bls_transit_stats* stats, qlp_bls_trapezoid* fits, qlp_bls_pink* pink,
+                     qlp_bls_star_grid* grid_out, int64_t* total_freq, void* cuda_stream);
+
 /* Release the context and its workspace.  NULL is allowed. */
 int qlp_bls_destroy(qlp_bls_ctx* ctx);
 

@@ -44,7 +44,7 @@ TRAP_DTYPE = np.dtype([("t0", "f8"), ("depth", "f8"), ("q", "f8"), ("q_in", "f8"
 PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8"), ("snr_pink", "f8"),
                        ("n_t", "i4"), ("n_transits", "i4"), ("n_bins", "i4"), ("detected", "i4")], align=True)
 
-EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
+EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_vet_host", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
            "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
@@ -71,6 +71,7 @@ def load_library():
         L.qlp_bls_trapezoid_fit.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_pink_noise.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_search_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
+        L.qlp_bls_vet_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), vp]
         L.qlp_bls_destroy.argtypes = [vp]
         L.qlp_bls_strerror.argtypes = [C.c_int]
         L.qlp_bls_strerror.restype = C.c_char_p
@@ -261,6 +262,23 @@ class QlpBls:
         if want_stats:
             return peaks.reshape(S, self.top_k), stats.reshape(S, self.top_k), grid, int(tf.value)
         return peaks.reshape(S, self.top_k), grid, int(tf.value)
+
+    def vet_host(self, row_ptr, t, y, dy, rho):
+        """qlp_bls_vet_host on numpy arrays -> (peaks, stats, fits, pink), structured [S, top_k] each: the search and
+        the rows after it from host buffers."""
+        S = int(row_ptr.shape[0]) - 1
+        n = S * self.top_k
+        peaks, stats = np.zeros(n, dtype=PEAK_DTYPE), np.zeros(n, dtype=STATS_DTYPE)
+        fits, pink = np.zeros(n, dtype=TRAP_DTYPE), np.zeros(n, dtype=PINK_DTYPE)
+        tf = C.c_int64()
+
+        def hp(a):
+            return C.c_void_p(a.ctypes.data)
+        _check(self.lib.qlp_bls_vet_host(self._h, S, hp(row_ptr), hp(t), hp(y), hp(dy), hp(rho), None, hp(peaks),
+                                         hp(stats), hp(fits), hp(pink), None, C.byref(tf), self._stream()),
+               "qlp_bls_vet_host")
+        shape = (S, self.top_k)
+        return peaks.reshape(shape), stats.reshape(shape), fits.reshape(shape), pink.reshape(shape)
 
     # -- test-only
     def debug_freqs(self, grid, star: int, k0: int, k1: int):

@@ -47,7 +47,7 @@ struct qlp_bls_ctx {
   // workspace
   DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work;
   // host-API staging
-  DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats;
+  DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats, h_fits, h_pink;
   static const int kSide = 3;           // side streams for the independent tile-class launches
   cudaStream_t side[kSide];
   cudaEvent_t side_done[kSide], fork_ev;
@@ -179,7 +179,7 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
                     &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
                     &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
-                    &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats};
+                    &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats, &ctx->h_fits, &ctx->h_pink};
   for (DevBuf* b : bufs) b->release();
   if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
   if (ctx->fork_ready) {
@@ -493,10 +493,10 @@ extern "C" int qlp_bls_pink_noise(qlp_bls_ctx* ctx, int64_t n_stars, const int64
 // sub-batch's copy is exposed.  Sub-batch size: enough points to keep the persistent fold kernels busy, small
 // enough for several sub-batches per call, and never more than a point budget that keeps the device copies
 // small next to 180 GB of HBM.
-extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
-                                   const double* y, const double* dy, const double* rho, const double* rstar,
-                                   qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_star_grid* grid_out,
-                                   int64_t* total_freq, void* cuda_stream) {
+static int search_host_impl(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                            const double* y, const double* dy, const double* rho, const double* rstar,
+                            qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_trapezoid* fits,
+                            qlp_bls_pink* pink, qlp_bls_star_grid* grid_out, int64_t* total_freq, void* cuda_stream) {
   (void)rstar;
   if (!ctx || n_stars < 0 || !row_ptr || !peaks) return QLP_BLS_EINVAL;
   if (n_stars > 0 && (!t || !y || !dy || !rho)) return QLP_BLS_EINVAL;
@@ -546,6 +546,8 @@ extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int6
   QLP_TRY(ctx->h_fptr.ensure((size_t)(max_S + 1) * 8));
   QLP_TRY(ctx->h_peaks.ensure((size_t)max_S * K * sizeof(qlp_bls_peak)));
   if (stats) QLP_TRY(ctx->h_stats.ensure((size_t)max_S * K * sizeof(qlp_bls_transit_stats)));
+  if (fits || pink) QLP_TRY(ctx->h_fits.ensure((size_t)max_S * K * sizeof(qlp_bls_trapezoid)));
+  if (pink) QLP_TRY(ctx->h_pink.ensure((size_t)max_S * K * sizeof(qlp_bls_pink)));
   int64_t* row_tmp[2] = {nullptr, nullptr};
   for (int i = 0; i < 2; ++i) {
     row_tmp[i] = (int64_t*)malloc((size_t)(max_S + 1) * 8);
@@ -607,8 +609,20 @@ extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int6
     if (rc == 0 && stats)
       rc = qlp_bls_peak_stats(ctx, S, d_row, d_t, d_y, d_dy, (const qlp_bls_peak*)ctx->h_peaks.p,
                               (qlp_bls_transit_stats*)ctx->h_stats.p, st);
+    if (rc == 0 && (fits || pink))   // synchronises the stream once (workspace sizing); the next H2D is already queued
+      rc = qlp_bls_trapezoid_fit(ctx, S, d_row, d_t, d_y, d_dy, (const qlp_bls_peak*)ctx->h_peaks.p,
+                                 (qlp_bls_trapezoid*)ctx->h_fits.p, st);
+    if (rc == 0 && pink)
+      rc = qlp_bls_pink_noise(ctx, S, d_row, d_t, d_y, (const qlp_bls_peak*)ctx->h_peaks.p,
+                              (const qlp_bls_trapezoid*)ctx->h_fits.p, (qlp_bls_pink*)ctx->h_pink.p, st);
     if (rc != 0) break;
     cudaError_t e = cudaEventRecord(ctx->set_free[set], st);
+    if (e == cudaSuccess && fits)
+      e = cudaMemcpyAsync(fits + cur.s0 * K, ctx->h_fits.p, (size_t)S * K * sizeof(qlp_bls_trapezoid),
+                          cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && pink)
+      e = cudaMemcpyAsync(pink + cur.s0 * K, ctx->h_pink.p, (size_t)S * K * sizeof(qlp_bls_pink),
+                          cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess && stats)
       e = cudaMemcpyAsync(stats + cur.s0 * K, ctx->h_stats.p, (size_t)S * K * sizeof(qlp_bls_transit_stats),
                           cudaMemcpyDeviceToHost, st);
@@ -628,6 +642,23 @@ extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int6
   if (rc == 0 && (e1 != cudaSuccess || e2 != cudaSuccess)) { cudaGetLastError(); rc = QLP_BLS_ECUDA; }
   if (rc == 0 && total_freq) *total_freq = tf_sum;
   return rc;
+}
+
+extern "C" int qlp_bls_search_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                   const double* y, const double* dy, const double* rho, const double* rstar,
+                                   qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_star_grid* grid_out,
+                                   int64_t* total_freq, void* cuda_stream) {
+  return search_host_impl(ctx, n_stars, row_ptr, t, y, dy, rho, rstar, peaks, stats, nullptr, nullptr, grid_out,
+                          total_freq, cuda_stream);
+}
+
+extern "C" int qlp_bls_vet_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                const double* y, const double* dy, const double* rho, const double* rstar,
+                                qlp_bls_peak* peaks, qlp_bls_transit_stats* stats, qlp_bls_trapezoid* fits,
+                                qlp_bls_pink* pink, qlp_bls_star_grid* grid_out, int64_t* total_freq,
+                                void* cuda_stream) {
+  return search_host_impl(ctx, n_stars, row_ptr, t, y, dy, rho, rstar, peaks, stats, fits, pink, grid_out, total_freq,
+                          cuda_stream);
 }
 
 // ---- test-only entry points ---------------------------------------------------------------------------

@@ -99,6 +99,22 @@ def test_pink_noise_sees_injected_red_noise_and_rejects_a_single_transit(gpu, or
         ctx.close()
 
 
+def test_vet_host_gives_the_same_bits_as_the_device_calls(gpu):
+    """qlp_bls_vet_host (host buffers, sub-batches) = grid -> spectrum -> snr -> peak_stats -> trapezoid_fit ->
+    pink_noise on device arrays: every kernel is deterministic and stars are independent."""
+    from paper_2302_01293_b200 import synth
+    b = synth.make_batch(5, star_ids=np.arange(24))
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        pk, fits, pink = run(gpu, ctx, b)
+        pk_h, st_h, ft_h, pn_h = ctx.vet_host(b.row_ptr, b.t, b.y, b.dy, b.rho)
+        assert pk_h.tobytes() == pk.tobytes()
+        assert ft_h.tobytes() == fits.tobytes() and pn_h.tobytes() == pink.tobytes()
+        assert st_h["n_in"].sum() > 0 and (ft_h["status"] == 0).any()
+    finally:
+        ctx.close()
+
+
 def test_pink_noise_empty_and_invalid(gpu):
     from paper_2302_01293_b200 import synth
     t = synth.sector_times(0, 1800.0)
