@@ -23,7 +23,7 @@ namespace qlp {
 
 constexpr int kFitWarps = 4;       // (star, peak) items per CTA of the counting kernel
 constexpr int kFitThreads = 256;   // threads of the CTA that fits one (star, peak)
-constexpr int kFitCap = 3072;      // points of a fit held in shared memory (72 KB: three CTAs per SM)
+constexpr int kFitCap = 2304;      // points of a fit held in shared memory (54 KB: four CTAs of 64 registers per SM)
 constexpr int kFitSmemBytes = 3 * kFitCap * 8;
 constexpr int kFitLevels = 24;     // step halvings
 constexpr int kFitMaxEval = 600;   // no sweep starts once this many chi2 evaluations are spent
@@ -181,7 +181,7 @@ __device__ __forceinline__ double trap_chi2(const FitData& fd, double* red3, int
   return chi2 > 0.0 ? chi2 : 0.0;
 }
 
-__global__ void __launch_bounds__(kFitThreads) fit_kernel(int64_t n_items, int top_k, const int64_t* __restrict__ row_ptr,
+__global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, int top_k, const int64_t* __restrict__ row_ptr,
                                                           const double* __restrict__ t, const double* __restrict__ y,
                                                           const double* __restrict__ dy,
                                                           const qlp_bls_peak* __restrict__ peaks,
