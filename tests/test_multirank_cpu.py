@@ -58,3 +58,18 @@ def test_reference_arm_other_ranks_do_nothing(monkeypatch, capsys):
     monkeypatch.setenv("RANK", "1")
     bench.run_reference(type("A", (), {"stars": 2, "config": 2, "steps": 1, "warmup": 0, "gpus": 2})())
     assert capsys.readouterr().out == ""
+
+
+def test_parallel_generation_reproduces_make_batch():
+    """bench.py --chunk builds each chunk from blocks of stars made by worker processes; every star has its own seed
+    (synth.make_star), so the packed chunk is the batch make_batch gives for the same ids."""
+    import multiprocessing
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2302_01293_b200 import synth
+    with multiprocessing.get_context("fork").Pool(2) as pool:
+        got = bench.make_workload_parallel(5, 7, 18, pool, block=4)
+    ref = synth.make_batch(5, star_ids=np.arange(7, 18))
+    for k in ("row_ptr", "t", "y", "dy", "rho", "rstar", "star_ids"):
+        assert np.array_equal(getattr(got, k), getattr(ref, k)), k
+    assert got.truth.tobytes() == ref.truth.tobytes()
