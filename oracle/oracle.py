@@ -20,7 +20,8 @@ _LIB = os.path.join(_HERE, "libqlp_oracle.so")
 class Config(C.Structure):
     _fields_ = [("samples_per_peak", C.c_double), ("dlogq", C.c_double), ("noverlap", C.c_int32),
                 ("pad_", C.c_int32), ("qmin_fac", C.c_double), ("qmax_fac", C.c_double),
-                ("a_over_rstar_min", C.c_double), ("sector_days", C.c_double)]
+                ("a_over_rstar_min", C.c_double), ("sector_days", C.c_double),
+                ("max_period_days", C.c_double), ("max_freq", C.c_int64)]
 
 
 GRID_DTYPE = np.dtype([("t_ref", "f8"), ("baseline", "f8"), ("p_min", "f8"), ("p_max", "f8"),
@@ -37,7 +38,7 @@ STATS_DTYPE = np.dtype([("n_in", "i4"), ("n_before", "i4"), ("n_after", "i4"), (
 
 def default_config(**kw) -> Config:
     """PAPER.md:19 (0.5-2.0 x q_circ), :23 (a = 2 R*), :35 (samples_per_peak=2, dlogq=0.1, noverlap=3), :7 (27.4 d)."""
-    c = Config(2.0, 0.1, 3, 0, 0.5, 2.0, 2.0, 27.4)
+    c = Config(2.0, 0.1, 3, 0, 0.5, 2.0, 2.0, 27.4, 0.0, 0)
     for k, v in kw.items():
         setattr(c, k, v)
     return c

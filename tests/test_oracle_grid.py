@@ -137,6 +137,52 @@ def test_grid_sizes_match_design(orc, cfg):
     assert 1e5 < orc.grid(cfg, t40, 1.0)["n_freq"] < 1.2e6
 
 
+def test_comparison_grid_caps(orc, cfg):
+    """O1.9: the earlier search's grid, "an under-sampled frequency grid on the order of 80,000
+    frequencies or less" with "periods up to only ~56 days".  Pins: caps that do not bite change nothing;
+    the period cap moves only the low-frequency end; the frequency cap keeps both ends and the f^(1/3) law
+    and stretches the step by (n - 1)/(M - 1)."""
+    t = 2000.0 + np.arange(0.0, 13 * 27.4, 1.0 / 48.0)          # 13 continuous sectors, 30-min cadence
+    g0 = orc.grid(cfg, t, 1.0)
+    n0 = int(g0["n_freq"])
+    assert g0["p_max"] == pytest.approx(0.5 * (t[-1] - t[0]), rel=1e-15) and g0["p_max"] > 56.0
+    # caps that do not bite: bit-identical descriptor
+    loose = orc.grid(orc.default_config(max_period_days=1e4, max_freq=n0), t, 1.0)
+    assert loose.tobytes() == g0.tobytes()
+    # period cap: P_max = 56 exactly, same step, same high end, fewer frequencies
+    gp = orc.grid(orc.default_config(max_period_days=56.0), t, 1.0)
+    assert gp["p_max"] == 56.0 and gp["h"] == g0["h"] and gp["p_min"] == g0["p_min"] and gp["c_q"] == g0["c_q"]
+    assert gp["u0"] == pytest.approx((1.0 / 56.0) ** (1.0 / 3.0), rel=1e-15)
+    assert gp["n_freq"] < n0 and gp["nb_max"] < g0["nb_max"]
+    # the dropped frequencies are exactly those below 1/56 (counted on the uncapped grid, +-1 for the offset)
+    f0, _ = orc.freqs(cfg, g0)
+    assert abs((n0 - int(gp["n_freq"])) - int(np.sum(f0 < 1.0 / 56.0))) <= 1
+    # frequency cap: exactly M frequencies over the same range
+    for M in (80000, 1000, 2):
+        cm = orc.default_config(max_freq=M)
+        gm = orc.grid(cm, t, 1.0)
+        if n0 <= M:
+            assert gm.tobytes() == g0.tobytes()
+            continue
+        assert gm["n_freq"] == M and gm["u0"] == g0["u0"] and gm["nb_max"] == g0["nb_max"]
+        u1 = (1.0 / g0["p_min"]) ** (1.0 / 3.0)
+        assert gm["h"] == pytest.approx((u1 - g0["u0"]) / (M - 1), rel=1e-14)
+        assert gm["h"] > g0["h"]                                 # under-sampled
+        f, nb = orc.freqs(cm, gm)
+        assert f.size == M and f[0] == f0[0]
+        assert f[-1] == pytest.approx(1.0 / g0["p_min"], rel=1e-13)
+        assert np.all(np.diff(f) > 0) and np.all(np.diff(nb) <= 0) and nb[-1] == 38
+        # uniform in u = f^(1/3)
+        du = np.diff(np.cbrt(f))
+        assert np.allclose(du, gm["h"], rtol=1e-9)
+    # both caps together = the comparison workload; a short light curve is untouched by it
+    both = orc.default_config(max_period_days=56.0, max_freq=80000)
+    t1, *_ = synth.make_star(1, 0)
+    assert orc.grid(both, t1, 1.0).tobytes() == orc.grid(cfg, t1, 1.0).tobytes()
+    gb = orc.grid(both, 2000.0 + np.arange(0.0, 13 * 27.4, 200.0 / 86400.0), 8.0)   # dense star, 200 s: > 80,000
+    assert gb["n_freq"] == 80000 and gb["p_max"] == 56.0
+
+
 def test_grid_invariances(orc, cfg):
     t, *_ = synth.make_star(3, 11)
     g = orc.grid(cfg, t, 1.7)
