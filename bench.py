@@ -137,11 +137,15 @@ def oracle_evals(orc, cfg, batch):
     return tot
 
 
+GRID_NOTE = "comparison grid O1.10 (PAPER.md:13): P <= 56 d, <= 80,000 frequencies per star"
+GRID_KW = {}   # --comparison-grid: the O1.10 caps, given to both the CUDA context and the oracle config
+
+
 def time_oracle(batch, n_stars: int, threads: int):
     """Run the oracle as it stands (OpenMP over stars) on the first n_stars -> (seconds, evals)."""
     from oracle import oracle as orc
     from paper_2302_01293_b200 import synth
-    cfg = orc.default_config()
+    cfg = orc.default_config(**GRID_KW)
     sub = synth.from_arrays([batch.star(s) for s in range(n_stars)], rho=batch.rho[:n_stars])
     ev = oracle_evals(orc, cfg, sub)
     t0 = time.perf_counter()
@@ -184,7 +188,8 @@ def run_reference(args):
     out = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
-           "config": {"workload": f"config{args.config}: {n}-star sample of BASELINE.json configs[{args.config - 1}]"},
+           "config": {"workload": f"config{args.config}: {n}-star sample of BASELINE.json configs[{args.config - 1}]",
+                      **({"grid": GRID_NOTE} if GRID_KW else {})},
            "stars_per_s": n * args.steps / tot_t,
            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                             "sample": f"{n} stars per step, {args.steps} steps"},
@@ -227,7 +232,7 @@ def run_gpu(args):
     if use_dist:
         dist.barrier()
     torch.cuda.set_device(local)
-    ctx = bls.QlpBls(device=local, top_k=3)
+    ctx = bls.QlpBls(device=local, top_k=3, **GRID_KW)
     # stars are independent: each rank searches its own shard, no data-path collective
     batch = make_workload(args.config, args.stars, rank)
     dev = bls.upload(batch, f"cuda:{local}")
@@ -325,7 +330,8 @@ def run_gpu(args):
         "config": {"workload": f"config{args.config}: BASELINE.json configs[{args.config - 1}], {S} stars per GPU, "
                                f"{int(batch.n_points)} points, {int(tf)} frequencies",
                    "l2": "inputs larger than L2 (no flush needed)" if batch.n_points * 24 > 126e6 else
-                         "inputs smaller than L2", "parallelism": f"stars sharded over {world} GPU(s), no collective"},
+                         "inputs smaller than L2", "parallelism": f"stars sharded over {world} GPU(s), no collective",
+                   **({"grid": GRID_NOTE} if GRID_KW else {})},
         "stars_per_s": stars_all * args.steps / (ms * 1e-3),
         "clocks": clocks,
         "e2e": {"value": evals_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -400,7 +406,7 @@ def run_full(args):
     build.build()
     pool = mp.get_context("fork").Pool(os.cpu_count() or 1)   # forked before the CUDA context exists
     torch.cuda.set_device(0)
-    ctx = bls.QlpBls(device=0, top_k=3)
+    ctx = bls.QlpBls(device=0, top_k=3, **GRID_KW)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     tot = {"ms": 0.0, "e2e_s": 0.0, "evals": 0, "points": 0, "freqs": 0, "bins": 0, "h2d": 0, "d2h": 0,
            "launches": 0, "gen_s": 0.0}
@@ -536,7 +542,12 @@ def main():
     ap.add_argument("--chunk", type=int, default=0,
                     help="search --stars stars in chunks of this many (one GPU; e.g. --config 5 --stars 200000 "
                          "--chunk 20000 is the whole production-shaped batch)")
+    ap.add_argument("--comparison-grid", action="store_true",
+                    help="search the comparison grid of DESIGN.md O1.10 (PAPER.md:13: periods up to 56 d, at most "
+                         "80,000 frequencies per star) instead of the paper's GPU grid")
     args = ap.parse_args()
+    if args.comparison_grid:
+        GRID_KW.update(max_period_days=56.0, max_freq=80000)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     _quiet_stdout()
     if args.impl == "reference":

@@ -69,6 +69,12 @@ typedef struct {
                                qlp_bls_spectrum, which then synchronises once); a violation makes
                                the call return QLP_BLS_EVALIDATION.  Other bits reserved (0)      */
   uint32_t reserved_;       /* 0                                                                 */
+  /* Comparison grid (O1.10; the earlier CPU search used "an under-sampled
+   * frequency grid on the order of 80,000 frequencies or less" and "periods up to only ~56 days").
+   * Both 0 (default) = the paper's GPU grid.  Only qlp_bls_grid reads them.                       */
+  double max_period_days;   /* > 0: P_max = min(P_max, max_period_days)                          */
+  int64_t max_freq;         /* >= 2: a star whose grid has more frequencies gets exactly max_freq
+                               of them over the same range, step (u1 - u0) / (max_freq - 1)      */
 } qlp_bls_config;
 
 /* Per-star grid descriptor, written by qlp_bls_grid() (device memory, one per star).

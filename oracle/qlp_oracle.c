@@ -42,7 +42,7 @@ typedef struct {
   double qmax_fac;         /* 2.0 */
   double a_over_rstar_min; /* 2.0 (3.0 for Sectors 59-60) */
   double sector_days;      /* 27.4 PAPER.md:7 */
-  /* O1.9, comparison grid only (the earlier search used "an under-sampled frequency grid on the
+  /* O1.10, comparison grid only (the earlier search used "an under-sampled frequency grid on the
    * order of 80,000 frequencies or less" and "periods up to only ~56 days").  0 = no cap (the paper's GPU grid). */
   double max_period_days;  /* 0, or e.g. 56.0 */
   int64_t max_freq;        /* 0, or e.g. 80000 */
@@ -127,7 +127,7 @@ void orc_grid(const orc_config* c, int64_t n, const double* t, double rho_in, or
     if (len > L) L = len;
   }
   double p_max = has_break ? L : 0.5 * L;
-  /* O1.9a: optional period cap of the comparison grid. */
+  /* O1.10a: optional period cap of the comparison grid. */
   if (c->max_period_days > 0.0 && p_max > c->max_period_days) p_max = c->max_period_days;
   g->p_max = p_max;
   /* O1.3: Kepler, a/R* = (G rho P^2 / 3 pi)^(1/3)  =>  P_min = sqrt(3 pi k^3 / (K_rho rho)). */
@@ -151,7 +151,7 @@ void orc_grid(const orc_config* c, int64_t n, const double* t, double rho_in, or
   double A = Q / (c->samples_per_peak * T);
   double h = A / 3.0;
   g->n_freq = (int64_t)floor((u1 - u0) / h) + 1;
-  /* O1.9b: optional cap on the number of frequencies: the same range in u, under-sampled to exactly max_freq
+  /* O1.10b: optional cap on the number of frequencies: the same range in u, under-sampled to exactly max_freq
    * points (step (u1 - u0) / (max_freq - 1)). */
   if (c->max_freq >= 2 && g->n_freq > c->max_freq) {
     h = (u1 - u0) / (double)(c->max_freq - 1);

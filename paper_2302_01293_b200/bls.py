@@ -24,7 +24,8 @@ class Config(C.Structure):
     _fields_ = [("struct_bytes", C.c_uint32), ("device", C.c_int32), ("samples_per_peak", C.c_double),
                 ("dlogq", C.c_double), ("noverlap", C.c_int32), ("top_k", C.c_int32),
                 ("qmin_fac", C.c_double), ("qmax_fac", C.c_double), ("a_over_rstar_min", C.c_double),
-                ("sector_days", C.c_double), ("flags", C.c_uint32), ("reserved_", C.c_uint32)]
+                ("sector_days", C.c_double), ("flags", C.c_uint32), ("reserved_", C.c_uint32),
+                ("max_period_days", C.c_double), ("max_freq", C.c_int64)]
 
 
 GRID_DTYPE = np.dtype([("t_ref", "f8"), ("baseline", "f8"), ("p_min", "f8"), ("p_max", "f8"),

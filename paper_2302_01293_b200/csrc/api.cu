@@ -116,7 +116,8 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
   if (cfg->struct_bytes != sizeof(qlp_bls_config)) return QLP_BLS_EINVAL;
   if (!(cfg->samples_per_peak > 0.0) || !(cfg->dlogq > 0.0) || cfg->noverlap < 1 || cfg->noverlap > kMaxWidth ||
       !(cfg->qmin_fac > 0.0) || !(cfg->qmax_fac >= cfg->qmin_fac) || !(cfg->a_over_rstar_min > 0.0) ||
-      !(cfg->sector_days > 0.0) || cfg->top_k < 1 || cfg->top_k > kMaxTopK)
+      !(cfg->sector_days > 0.0) || cfg->top_k < 1 || cfg->top_k > kMaxTopK ||
+      !(cfg->max_period_days >= 0.0) || cfg->max_freq < 0 || cfg->max_freq == 1)
     return QLP_BLS_EINVAL;
   qlp_bls_ctx* ctx = new (std::nothrow) qlp_bls_ctx();
   if (!ctx) return QLP_BLS_ENOMEM;
@@ -127,6 +128,7 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
   p.samples_per_peak = cfg->samples_per_peak; p.dlogq = cfg->dlogq; p.qmin_fac = cfg->qmin_fac;
   p.qmax_fac = cfg->qmax_fac; p.a_over_rstar_min = cfg->a_over_rstar_min; p.sector_days = cfg->sector_days;
   p.noverlap = cfg->noverlap; p.top_k = cfg->top_k;
+  p.max_period_days = cfg->max_period_days; p.max_freq = cfg->max_freq;
   p.wmask = 0; p.max_width = 0; p.min_width = ctx->widths[0];
   for (int i = 0; i < ctx->n_widths; ++i) {
     int m = ctx->widths[i];

@@ -45,6 +45,8 @@ struct StarPrep {
 // Resolved search parameters (device copy of qlp_bls_config plus derived values).
 struct Params {
   double samples_per_peak, dlogq, qmin_fac, qmax_fac, a_over_rstar_min, sector_days;
+  double max_period_days;  // O1.10a: 0 = no period cap
+  int64_t max_freq;        // O1.10b: 0 = no cap on the number of frequencies
   int32_t noverlap, top_k;
   uint32_t wmask;     // bit m set <=> width m is on the ladder (O1.9)
   int32_t max_width;  // largest width

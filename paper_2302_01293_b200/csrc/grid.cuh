@@ -80,6 +80,8 @@ __global__ void __launch_bounds__(256) grid_kernel(Params prm, int64_t n_stars, 
         if (len > L) L = len;
       }
       double p_max = has_break ? L : dmul(0.5, L);
+      // O1.10a: period cap of the comparison grid
+      if (prm.max_period_days > 0.0 && p_max > prm.max_period_days) p_max = prm.max_period_days;
       q.p_max = p_max;
       // O1.3: a/R* = (G rho P^2 / 3 pi)^(1/3)  =>  P_min = sqrt(3 pi k^3 / (K_rho rho))
       double D = dmul(QLP_K_RHO, rh);
@@ -100,8 +102,13 @@ __global__ void __launch_bounds__(256) grid_kernel(Params prm, int64_t n_stars, 
           double Q = dmul(prm.qmin_fac, q.c_q);
           double A = ddiv(Q, dmul(prm.samples_per_peak, T));
           double h = ddiv(A, 3.0);
-          q.u0 = u0; q.h = h;
           q.n_freq = (int64_t)floor(ddiv(dsub(u1, u0), h)) + 1;
+          // O1.10b: at most max_freq frequencies over the same range in u (under-sampled comparison grid)
+          if (prm.max_freq >= 2 && q.n_freq > prm.max_freq) {
+            h = ddiv(dsub(u1, u0), (double)(prm.max_freq - 1));
+            q.n_freq = prm.max_freq;
+          }
+          q.u0 = u0; q.h = h;
           double qlo = dmul(Q, dmul(u0, u0));
           q.nb_max = (int32_t)ceil(ddiv((double)prm.noverlap, qlo));
           if (q.nb_max > QLP_BLS_MAX_NB || q.nb_max <= 0) { q.status = 4; q.n_freq = 0; }

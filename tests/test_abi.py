@@ -38,10 +38,11 @@ def test_struct_layouts(lib):
     assert bls.PEAK_DTYPE.itemsize == 64
     assert bls.STATS_DTYPE.itemsize == 32 and bls.TRAP_DTYPE.itemsize == 72 and bls.PINK_DTYPE.itemsize == 48
     cfg = bls.default_config()
-    assert cfg.struct_bytes == C.sizeof(bls.Config) == 72
+    assert cfg.struct_bytes == C.sizeof(bls.Config) == 88
     # the paper's parameters: PAPER.md:35 (samples_per_peak=2, dlogq=0.1, noverlap=3), :19, :23, :7
     assert (cfg.samples_per_peak, cfg.dlogq, cfg.noverlap) == (2.0, 0.1, 3)
     assert (cfg.qmin_fac, cfg.qmax_fac, cfg.a_over_rstar_min, cfg.sector_days) == (0.5, 2.0, 2.0, 27.4)
+    assert (cfg.max_period_days, cfg.max_freq) == (0.0, 0)       # the paper's GPU grid: no caps (O1.10)
 
 
 def test_strerror_and_bad_args(lib):
@@ -53,6 +54,8 @@ def test_strerror_and_bad_args(lib):
     cfg = bls.default_config(top_k=99)
     h = C.c_void_p()
     assert lib.qlp_bls_create(C.byref(cfg), C.byref(h)) == -1
+    for bad in (dict(max_freq=1), dict(max_freq=-5), dict(max_period_days=-1.0)):
+        assert lib.qlp_bls_create(C.byref(bls.default_config(**bad)), C.byref(h)) == -1
     cfg = bls.default_config(a_over_rstar_min=0.5)  # boxes would be wider than the histogram
     assert lib.qlp_bls_create(C.byref(cfg), C.byref(h)) == -1
     assert lib.qlp_bls_destroy(None) == 0

@@ -317,10 +317,40 @@ def test_constant_and_degenerate_light_curves(gpu, ctx, orc, cfg):
         assert np.abs(sr[fp[s]:fp[s + 1]] - so).max() <= SR_RTOL * so.max()
 
 
+def test_comparison_grid_long_baseline(gpu, orc):
+    """O1.10 with the values PAPER.md:13 quotes (56 d, 80,000 frequencies) on 13-sector stars (config 4): descriptors
+    and sampled (f_k, nb_k) bit-exact, the period cap biting on every star."""
+    from paper_2302_01293_b200 import synth
+    kw = dict(max_period_days=56.0, max_freq=80000)
+    ocfg = orc.default_config(**kw)
+    b = synth.make_batch(4, n_stars=4)
+    ctx = gpu.QlpBls(**kw)
+    free = gpu.QlpBls()
+    try:
+        dev = gpu.upload(b)
+        grid, freq_ptr, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        gg = gpu.grid_to_numpy(grid)
+        go = _oracle_grids(orc, ocfg, b)
+        _assert_grid_equal(gg, go)
+        g_free = gpu.grid_to_numpy(free.grid(dev[0], dev[1], dev[4], dev[5])[0])
+        assert np.all(gg["p_max"] == 56.0) and np.all(g_free["p_max"] > 56.0)
+        assert np.all(gg["n_freq"] <= 80000) and np.all(gg["n_freq"] < g_free["n_freq"])
+        assert int(tf) == int(gg["n_freq"].sum())
+        for s in range(b.n_stars):
+            n = int(gg["n_freq"][s])
+            for k0 in (0, n // 2, max(0, n - 64)):
+                f, nb = ctx.debug_freqs(grid, s, k0, min(n, k0 + 64))
+                fo, nbo = orc.freqs(ocfg, go[s], k0, min(n, k0 + 64))
+                assert np.array_equal(f.cpu().numpy(), fo) and np.array_equal(nb.cpu().numpy(), nbo)
+    finally:
+        ctx.close(); free.close()
+
+
 @pytest.mark.parametrize("kw", [dict(a_over_rstar_min=3.0),                       # Sectors 59-60 variant, PAPER.md:23
                                 dict(noverlap=4, dlogq=0.2),                       # ladder {4,5,6,7,8,10,12,14}: gaps, width 14
                                 dict(noverlap=2, qmax_fac=3.0),                    # ladder {2..11}
-                                dict(noverlap=5, dlogq=0.05, qmax_fac=1.5)])       # ladder {5..15}
+                                dict(noverlap=5, dlogq=0.05, qmax_fac=1.5),        # ladder {5..15}
+                                dict(max_period_days=5.0, max_freq=1500)])         # O1.10 caps, both biting on config 2
 def test_other_search_parameters(gpu, orc, kw):
     """Non-default qlp_bls_config: grid bit-exact and SR parity with the oracle under the same parameters.
     Ladders other than the paper's {3..11} run the generic (run-time mask, 16-wide window) kernel."""

@@ -138,7 +138,7 @@ def test_grid_sizes_match_design(orc, cfg):
 
 
 def test_comparison_grid_caps(orc, cfg):
-    """O1.9: the earlier search's grid, "an under-sampled frequency grid on the order of 80,000
+    """O1.10: the earlier search's grid, "an under-sampled frequency grid on the order of 80,000
     frequencies or less" with "periods up to only ~56 days".  Pins: caps that do not bite change nothing;
     the period cap moves only the low-frequency end; the frequency cap keeps both ends and the f^(1/3) law
     and stretches the step by (n - 1)/(M - 1)."""
