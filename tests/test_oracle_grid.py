@@ -181,6 +181,11 @@ def test_comparison_grid_caps(orc, cfg):
     assert orc.grid(both, t1, 1.0).tobytes() == orc.grid(cfg, t1, 1.0).tobytes()
     gb = orc.grid(both, 2000.0 + np.arange(0.0, 13 * 27.4, 200.0 / 86400.0), 8.0)   # dense star, 200 s: > 80,000
     assert gb["n_freq"] == 80000 and gb["p_max"] == 56.0
+    # context of PAPER.md:59 ("up to ~10 times more frequencies" on the GPU grid): longest baseline (40 sectors),
+    # a dense (rho* = 10) star; a solar star gets ~3 times more, a single-sector star the same grid
+    t40 = 2000.0 + np.arange(0.0, 40 * 27.4, 1.0 / 48.0)
+    ratio = lambda rho: orc.grid(cfg, t40, rho)["n_freq"] / orc.grid(both, t40, rho)["n_freq"]
+    assert 5.0 < ratio(10.0) < 15.0 and 2.0 < ratio(1.0) < 4.0
 
 
 def test_grid_invariances(orc, cfg):
