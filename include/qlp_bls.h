@@ -71,7 +71,8 @@ typedef struct {
   uint32_t reserved_;       /* 0                                                                 */
   /* Comparison grid (O1.10; the earlier CPU search used "an under-sampled
    * frequency grid on the order of 80,000 frequencies or less" and "periods up to only ~56 days").
-   * Both 0 (default) = the paper's GPU grid.  Only qlp_bls_grid reads them.                       */
+   * Both 0 (default) = the paper's GPU grid.  Only qlp_bls_grid reads them.  qlp_bls_create returns
+   * QLP_BLS_EINVAL for max_period_days < 0 (or NaN), max_freq < 0 or max_freq == 1.              */
   double max_period_days;   /* > 0: P_max = min(P_max, max_period_days)                          */
   int64_t max_freq;         /* >= 2: a star whose grid has more frequencies gets exactly max_freq
                                of them over the same range, step (u1 - u0) / (max_freq - 1)      */
