@@ -93,7 +93,9 @@ typedef struct {
   int32_t nb_max;   /* phase bins at k = 0 (the largest)                                         */
   int32_t status;   /* 0 ok; 1 fewer than 2 points; 2 baseline <= 0; 3 f_max <= f_min;
                        4 nb_max > QLP_BLS_MAX_NB (star skipped, n_freq = 0);
-                       5 more than QLP_BLS_MAX_POINTS points (star skipped, n_freq = 0)           */
+                       5 more than QLP_BLS_MAX_POINTS points (star skipped, n_freq = 0);
+                       7 timestamps not finite and strictly increasing (star skipped, n_freq = 0:
+                         checked for every star, whether or not flags bit0 asks for validation)    */
 } qlp_bls_star_grid;
 
 /* One peak of one star, written by qlp_bls_snr() (device memory, [S * top_k], rank-major within
@@ -195,7 +197,11 @@ int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, 
  * sigma = 1.4826 MAD; bin count by Sturges' law, footnote 3 at :65) and the top_k peaks with
  * period, epoch, depth, duration.  DESIGN.md O5-O6.
  *   in : as qlp_bls_spectrum plus its outputs sr, best.
- *   out: snr dev float[total_freq] or NULL; peaks dev [S * top_k]. */
+ *   out: snr dev float[total_freq] or NULL; peaks dev [S * top_k].
+ * The prepared point records of the last qlp_bls_spectrum call of this context are reused when this call names
+ * the same arrays (row_ptr, t, y, dy, grid pointers and n_stars) and no other call of the context touched the
+ * workspace in between; otherwise S0 is run again.  The caller must not rewrite those arrays in place between
+ * the two calls. */
 int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                 const double* y, const double* dy, const qlp_bls_star_grid* grid,
                 const int64_t* freq_ptr, const float* sr, const uint32_t* best, float* snr,
@@ -263,6 +269,11 @@ int qlp_bls_fold_elapsed_ms(qlp_bls_ctx* ctx, int32_t* n_calls /*host*/, double*
  * clocks[0] = tile set-up + zeroing, clocks[1] = fold (S2), clocks[2] = box scan + reduction + output (S3).
  * Their ratios split the fused kernel's time between S2 and S3.  Synchronises the device.  clocks host [3]. */
 int qlp_bls_fold_phase_clocks(qlp_bls_ctx* ctx, uint64_t* clocks /*host*/);
+
+/* Per tile class c = 0..8 of the fold/scan kernel, summed over all tiles since
+ * qlp_bls_fold_timing(ctx, 1): out host uint64[9][5] = {set-up + zeroing clocks, fold clocks, scan clocks (SM clocks
+ * of thread 0 of each CTA), point x frequency evaluations, tiles}.  Synchronises the device. */
+int qlp_bls_fold_class_counters(qlp_bls_ctx* ctx, uint64_t* out);
 
 /* The duration ladder in fine bins (O1.9): writes up to cap widths to m (host),
  * returns their number. */

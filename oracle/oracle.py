@@ -160,6 +160,34 @@ def spectrum_star(cfg: Config, g, t, y, dy):
     return sr, m, j
 
 
+def spectrum_samples(cfg: Config, g, t, y, dy, ks):
+    """O3+O4 of one star at the grid indices ks (OpenMP over the samples) -> (sr, m, j)."""
+    t, y, dy = _f8(t), _f8(y), _f8(dy)
+    ga = np.array([g], dtype=GRID_DTYPE)
+    ks = np.ascontiguousarray(ks, dtype=np.int64)
+    sr = np.zeros(ks.size)
+    m = np.zeros(ks.size, dtype=np.int32)
+    j = np.zeros(ks.size, dtype=np.int32)
+    rc = lib().orc_spectrum_samples(C.byref(cfg), _p(ga), C.c_int64(t.size), _p(t), _p(y), _p(dy),
+                                    C.c_int64(ks.size), _p(ks), _p(sr), _p(m), _p(j))
+    assert rc == 0, rc
+    return sr, m, j
+
+
+def box_values(cfg: Config, g, t, y, dy, ks, ms, js) -> np.ndarray:
+    """Value s^2/(r(1-r)) of the given boxes (ms bins from start bin js) at grid indices ks, oracle arithmetic."""
+    t, y, dy = _f8(t), _f8(y), _f8(dy)
+    ga = np.array([g], dtype=GRID_DTYPE)
+    ks = np.ascontiguousarray(ks, dtype=np.int64)
+    ms = np.ascontiguousarray(ms, dtype=np.int32)
+    js = np.ascontiguousarray(js, dtype=np.int32)
+    val = np.zeros(ks.size)
+    rc = lib().orc_box_values(C.byref(cfg), _p(ga), C.c_int64(t.size), _p(t), _p(y), _p(dy),
+                              C.c_int64(ks.size), _p(ks), _p(ms), _p(js), _p(val))
+    assert rc == 0, rc
+    return val
+
+
 def snr(f, sr):
     """O5 -> (snr, trend, sigma)."""
     f, sr = _f8(f), _f8(sr)

@@ -280,6 +280,67 @@ int orc_spectrum_star(const orc_config* c, const orc_star_grid* g, int64_t n, co
   return 0;
 }
 
+/* Test helpers (no new arithmetic: they only call orc_prep / orc_freq / orc_sr_one / orc_bin1 above).
+ * orc_spectrum_samples: O3+O4 of one star at the selected grid indices ks[0..nk), OpenMP over the samples, so that
+ * long-baseline stars (10^5..10^6 frequencies) can be checked on a sample.  r_best/s_best optional (NULL). */
+int orc_spectrum_samples(const orc_config* c, const orc_star_grid* g, int64_t n, const double* t, const double* y,
+                         const double* dy, int64_t nk, const int64_t* ks, double* sr, int32_t* m_best,
+                         int32_t* j_best) {
+  if (g->status != 0 || g->n_freq <= 0 || nk <= 0) return 0;
+  int32_t M[ORC_MAX_WIDTHS];
+  int nM = orc_widths(c, M);
+  if (nM <= 0) return -1;
+  double* tau = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1) * 3);
+  if (!tau) return -2;
+  double* w = tau + n;
+  double* wy = w + n;
+  orc_prep(n, t, y, dy, g->t_ref, tau, w, wy);
+  int err = 0;
+#pragma omp parallel
+  {
+    double* Hw = (double*)malloc(sizeof(double) * (size_t)g->nb_max * 2);
+    if (!Hw) err = -2;
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t i = 0; i < nk; ++i) {
+      if (!Hw || ks[i] < 0 || ks[i] >= g->n_freq) { if (Hw) err = -3; continue; }
+      double f; int32_t nb;
+      orc_freq(c, g, ks[i], &f, &nb);
+      orc_sr_one(n, tau, w, wy, f, nb, nM, M, Hw, Hw + g->nb_max, &sr[i], &m_best[i], &j_best[i], NULL, NULL);
+    }
+    free(Hw);
+  }
+  free(tau);
+  return err;
+}
+
+/* orc_box_values: the value s^2 / (r (1 - r)) (0 outside 0 < r < 1) of GIVEN boxes (ms[i] bins from start bin
+ * js[i], wrapped) at grid indices ks[i] of one star: lets a test check that a box reported by another
+ * implementation is as good as the oracle's best one.  Sums run over the points in time order. */
+int orc_box_values(const orc_config* c, const orc_star_grid* g, int64_t n, const double* t, const double* y,
+                   const double* dy, int64_t nk, const int64_t* ks, const int32_t* ms, const int32_t* js,
+                   double* val) {
+  if (g->status != 0 || g->n_freq <= 0 || nk <= 0) return 0;
+  double* tau = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1) * 3);
+  if (!tau) return -2;
+  double* w = tau + n;
+  double* wy = w + n;
+  orc_prep(n, t, y, dy, g->t_ref, tau, w, wy);
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t i = 0; i < nk; ++i) {
+    double f; int32_t nb;
+    orc_freq(c, g, ks[i], &f, &nb);
+    double r = 0.0, s = 0.0;
+    for (int64_t p = 0; p < n; ++p) {
+      int32_t d = orc_bin1(f, nb, tau[p]) - js[i];
+      if (d < 0) d += nb;
+      if (d < ms[i]) { r += w[p]; s += wy[p]; }
+    }
+    val[i] = (r > 0.0 && r < 1.0) ? (s * s) / (r * (1.0 - r)) : 0.0;
+  }
+  free(tau);
+  return 0;
+}
+
 /* ---------------------------------------------------------------- O5 */
 static int cmp_double(const void* a, const void* b) {
   double x = *(const double*)a, y = *(const double*)b;

@@ -47,7 +47,7 @@ PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8")
 
 EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_vet_host", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
-           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
+           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_fold_class_counters", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path"]
 
 _lib = None
@@ -86,6 +86,7 @@ def load_library():
         L.qlp_bls_fold_timing.argtypes = [vp, i32]
         L.qlp_bls_fold_elapsed_ms.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_double)]
         L.qlp_bls_fold_phase_clocks.argtypes = [vp, vp]
+        L.qlp_bls_fold_class_counters.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -165,6 +166,13 @@ class QlpBls:
         a = np.zeros(3, dtype=np.uint64)
         _check(self.lib.qlp_bls_fold_phase_clocks(self._h, a.ctypes.data_as(C.c_void_p)), "qlp_bls_fold_phase_clocks")
         return [int(x) for x in a]
+
+    def fold_class_counters(self) -> np.ndarray:
+        """-> uint64[9, 5]: per tile class (set-up, fold, scan clocks of thread 0; evaluations; tiles)."""
+        a = np.zeros((9, 5), dtype=np.uint64)
+        _check(self.lib.qlp_bls_fold_class_counters(self._h, a.ctypes.data_as(C.c_void_p)),
+               "qlp_bls_fold_class_counters")
+        return a
 
     def debug_set_path(self, path: int):
         _check(self.lib.qlp_bls_debug_set_path(self._h, path), "qlp_bls_debug_set_path")

@@ -18,6 +18,7 @@
 
 using namespace qlp;
 
+static constexpr int kClassCtr = 8;  // uint64 counters per tile class (5 used), see qlp_bls_fold_class_counters
 static constexpr uint32_t kPaperMask = 0xFF8u;  // widths 3..11 (PAPER.md:19, :35 -> DESIGN.md O1.9)
 
 struct DevBuf {
@@ -47,7 +48,7 @@ struct qlp_bls_ctx {
   int32_t force_path = 0;
   int64_t launches = 0;
   // workspace
-  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work;
+  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work, class_ctr;
   // host-API staging
   DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats, h_fits, h_pink;
   static const int kSide = 3;           // side streams for the independent tile-class launches
@@ -58,9 +59,20 @@ struct qlp_bls_ctx {
   cudaEvent_t h2d_done[2], set_free[2];
   bool copy_ready = false;
   int64_t* totals_host = nullptr;  // pinned, 4 x int64
-  // cache of the last grid call: lets spectrum/snr size the point workspace without a sync
-  const int64_t* last_row_ptr = nullptr;
-  int64_t last_n_stars = -1, last_n_points = -1;
+  // The prepared point records (S0) in `pts` / `prep` belong to the arrays of the last run_prep call; qlp_bls_snr
+  // reuses them only if it is given the same arrays and nothing else wrote the workspace since.
+  struct PrepKey {
+    const void *row_ptr = nullptr, *t = nullptr, *y = nullptr, *dy = nullptr, *grid = nullptr;
+    int64_t n_stars = -1;
+    bool operator==(const PrepKey& o) const {
+      return row_ptr == o.row_ptr && t == o.t && y == o.y && dy == o.dy && grid == o.grid && n_stars == o.n_stars;
+    }
+  } prep_key;
+  bool prep_valid = false;
+  const void* grid_row_ptr = nullptr;  // batch of the last qlp_bls_grid call: only the test-only debug_prep call
+  int64_t grid_n_stars = -1;           // reads it (to learn the batch size); no workspace is sized from it
+  int64_t* row_tmp[2] = {nullptr, nullptr};   // pinned staging of the rebased row_ptr of a host sub-batch
+  size_t row_tmp_cap = 0;
   // optional per-call CUDA-event timing of the fold/scan launches (bench.py's roofline figure)
   static const int kRing = 256;
   bool timing = false;
@@ -181,11 +193,12 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   if (!ctx) return QLP_BLS_OK;
   cudaSetDevice(ctx->device);
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
-                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
+                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->class_ctr, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
                     &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats, &ctx->h_fits, &ctx->h_pink};
   for (DevBuf* b : bufs) b->release();
   if (ctx->totals_host) cudaFreeHost(ctx->totals_host);
+  for (int i = 0; i < 2; ++i) if (ctx->row_tmp[i]) cudaFreeHost(ctx->row_tmp[i]);
   if (ctx->fork_ready) {
     for (int i = 0; i < qlp_bls_ctx::kSide; ++i) { cudaStreamDestroy(ctx->side[i]); cudaEventDestroy(ctx->side_done[i]); }
     cudaEventDestroy(ctx->fork_ev);
@@ -233,15 +246,31 @@ extern "C" int qlp_bls_fold_timing(qlp_bls_ctx* ctx, int32_t enable) {
   }
   ctx->timing = enable != 0;
   ctx->ev_calls = 0;
-  CUDA_TRY(cudaMemset((unsigned long long*)ctx->totals_dev.p + 4, 0, 3 * 8));
+  QLP_TRY(ctx->class_ctr.ensure(kNumClasses * kClassCtr * 8));
+  CUDA_TRY(cudaMemset(ctx->class_ctr.p, 0, kNumClasses * kClassCtr * 8));
+  return QLP_BLS_OK;
+}
+
+extern "C" int qlp_bls_fold_class_counters(qlp_bls_ctx* ctx, uint64_t* out) {
+  if (!ctx || !out) return QLP_BLS_EINVAL;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  if (!ctx->class_ctr.p) { memset(out, 0, kNumClasses * 5 * 8); return QLP_BLS_OK; }
+  unsigned long long h[kNumClasses * kClassCtr];
+  CUDA_TRY(cudaDeviceSynchronize());
+  CUDA_TRY(cudaMemcpy(h, ctx->class_ctr.p, sizeof(h), cudaMemcpyDeviceToHost));
+  for (int c = 0; c < kNumClasses; ++c)
+    for (int i = 0; i < 5; ++i) out[c * 5 + i] = h[c * kClassCtr + i];
   return QLP_BLS_OK;
 }
 
 extern "C" int qlp_bls_fold_phase_clocks(qlp_bls_ctx* ctx, uint64_t* clocks) {
   if (!ctx || !clocks) return QLP_BLS_EINVAL;
-  CUDA_TRY(cudaSetDevice(ctx->device));
-  CUDA_TRY(cudaDeviceSynchronize());
-  CUDA_TRY(cudaMemcpy(clocks, (unsigned long long*)ctx->totals_dev.p + 4, 3 * 8, cudaMemcpyDeviceToHost));
+  uint64_t all[kNumClasses * 5];
+  QLP_TRY(qlp_bls_fold_class_counters(ctx, all));
+  for (int i = 0; i < 3; ++i) {
+    clocks[i] = 0;
+    for (int c = 0; c < kNumClasses; ++c) clocks[i] += all[c * 5 + i];
+  }
   return QLP_BLS_OK;
 }
 
@@ -301,24 +330,19 @@ extern "C" int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* ro
   freq_scan_kernel<<<1, 1024, 0, st>>>(n_stars, grid, (const unsigned long long*)ctx->star_bins.p, freq_ptr, totals);
   QLP_TRY(launch_ok(ctx));
   CUDA_TRY(cudaMemcpyAsync(ctx->totals_host, totals, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 2, row_ptr + n_stars, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   *total_freq = ctx->totals_host[0];
   *total_bins = ctx->totals_host[1];
-  ctx->last_row_ptr = row_ptr; ctx->last_n_stars = n_stars; ctx->last_n_points = ctx->totals_host[2];
+  ctx->grid_row_ptr = row_ptr; ctx->grid_n_stars = n_stars;
   return QLP_BLS_OK;
 }
 
-// number of points of the batch: cached by qlp_bls_grid, else one small synchronising read-back
+// number of points of the batch: always read from the device (8 bytes, one stream synchronisation).  The workspace
+// is sized from it, so nothing cached under a pointer that a caching allocator may hand out again is trusted.
 static int batch_points(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, cudaStream_t st, int64_t* n_points) {
-  if (ctx->last_row_ptr == row_ptr && ctx->last_n_stars == n_stars && ctx->last_n_points >= 0) {
-    *n_points = ctx->last_n_points;
-    return 0;
-  }
   CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 2, row_ptr + n_stars, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   *n_points = ctx->totals_host[2];
-  ctx->last_row_ptr = row_ptr; ctx->last_n_stars = n_stars; ctx->last_n_points = *n_points;
   return 0;
 }
 
@@ -326,13 +350,19 @@ static int batch_points(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_pt
 static int run_prep(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
                     const double* dy, const qlp_bls_star_grid* grid, cudaStream_t st) {
   int64_t n_points = 0;
+  ctx->prep_valid = false;
   QLP_TRY(batch_points(ctx, n_stars, row_ptr, st, &n_points));
   if (n_points < 0) return QLP_BLS_EINVAL;
   QLP_TRY(ctx->pts.ensure((size_t)(n_points + 1) * sizeof(Point)));
   QLP_TRY(ctx->prep.ensure((size_t)(n_stars + 1) * sizeof(StarPrep)));
   prep_kernel<<<(unsigned)n_stars, 256, 0, st>>>(ctx->prm, n_stars, row_ptr, t, y, dy, grid, (Point*)ctx->pts.p,
                                                 (StarPrep*)ctx->prep.p);
-  return launch_ok(ctx);
+  QLP_TRY(launch_ok(ctx));
+  qlp_bls_ctx::PrepKey k;
+  k.row_ptr = row_ptr; k.t = t; k.y = y; k.dy = dy; k.grid = grid; k.n_stars = n_stars;
+  ctx->prep_key = k;
+  ctx->prep_valid = true;
+  return 0;
 }
 
 // ---- S0 + S2 + S3 ---------------------------------------------------------------------------------
@@ -357,7 +387,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   unsigned long long* counters = (unsigned long long*)ctx->counters.p;
   CUDA_TRY(cudaMemsetAsync(counters, 0, kNumClasses * 8, st));
   // per-phase clock counters of the fold/scan kernel (only while fold timing is on)
-  unsigned long long* phase = ctx->timing ? (unsigned long long*)ctx->totals_dev.p + 4 : nullptr;
+  unsigned long long* phase_base = (ctx->timing && ctx->class_ctr.p) ? (unsigned long long*)ctx->class_ctr.p : nullptr;
   tile_bounds_kernel<<<(unsigned)((n_stars + 127) / 128), 128, 0, st>>>(ctx->prm, n_stars, grid, ctx->force_path, kb, cnt);
   QLP_TRY(launch_ok(ctx));
   tile_scan_kernel<<<kNumClasses, 1024, 0, st>>>(n_stars, cnt, off);
@@ -387,7 +417,8 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
 #define QLP_LAUNCH(MW_, CT_, WM_)                                                                                          \
   foldscan_kernel<MW_, CT_, WM_><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,    \
                                                          (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,    \
-                                                         counters + c, sr, best, phase)
+                                                         counters + c, sr, best,                               \
+                                                         phase_base ? phase_base + c * kClassCtr : nullptr)
 #define QLP_LAUNCH_MW(CT_) do { if (generic) QLP_LAUNCH(16, CT_, 0u); else QLP_LAUNCH(11, CT_, kPaperMask); } while (0)
     switch (class_cols(c)) {
       case 128: QLP_LAUNCH_MW(128); break;
@@ -420,7 +451,11 @@ extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row
   if (n_stars > 0x7fffffff) return QLP_BLS_EUNSUPPORTED;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(ctx->device));
-  QLP_TRY(run_prep(ctx, n_stars, row_ptr, t, y, dy, grid, st));  // one cheap pass; never trusts stale state
+  {  // S0 again only if the workspace does not hold these arrays' records (see the header)
+    qlp_bls_ctx::PrepKey k;
+    k.row_ptr = row_ptr; k.t = t; k.y = y; k.dy = dy; k.grid = grid; k.n_stars = n_stars;
+    if (!(ctx->prep_valid && ctx->prep_key == k)) QLP_TRY(run_prep(ctx, n_stars, row_ptr, t, y, dy, grid, st));
+  }
   snr_kernel<<<(unsigned)n_stars, kSnrThreads, kMaxSel * 256 * 4, st>>>(
       ctx->prm, n_stars, row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, grid, freq_ptr, sr, best,
       snr, peaks);
@@ -556,11 +591,19 @@ static int search_host_impl(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* ro
   if (stats) QLP_TRY(ctx->h_stats.ensure((size_t)max_S * K * sizeof(qlp_bls_transit_stats)));
   if (fits || pink) QLP_TRY(ctx->h_fits.ensure((size_t)max_S * K * sizeof(qlp_bls_trapezoid)));
   if (pink) QLP_TRY(ctx->h_pink.ensure((size_t)max_S * K * sizeof(qlp_bls_pink)));
-  int64_t* row_tmp[2] = {nullptr, nullptr};
-  for (int i = 0; i < 2; ++i) {
-    row_tmp[i] = (int64_t*)malloc((size_t)(max_S + 1) * 8);
-    if (!row_tmp[i]) { free(row_tmp[0]); return QLP_BLS_ENOMEM; }
+  // pinned, so that the copy stream's H2D of the rebased row_ptr is asynchronous like the others
+  if (ctx->row_tmp_cap < (size_t)(max_S + 1)) {
+    for (int i = 0; i < 2; ++i) {
+      if (ctx->row_tmp[i]) cudaFreeHost(ctx->row_tmp[i]);
+      ctx->row_tmp[i] = nullptr;
+    }
+    ctx->row_tmp_cap = 0;
+    const size_t want = (size_t)(max_S + 1) + (size_t)(max_S + 1) / 8;
+    for (int i = 0; i < 2; ++i)
+      if (cudaMallocHost((void**)&ctx->row_tmp[i], want * 8) != cudaSuccess) { cudaGetLastError(); return QLP_BLS_ENOMEM; }
+    ctx->row_tmp_cap = want;
   }
+  int64_t** row_tmp = ctx->row_tmp;
   struct Sub { int64_t s0, s1; };
   int64_t sub_idx = 0;
   auto next_sub = [&](int64_t) { const Sub sb{cut[sub_idx], cut[sub_idx + 1]}; ++sub_idx; return sb; };
@@ -598,7 +641,7 @@ static int search_host_impl(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* ro
     const double* d_y = (const double*)ctx->h_y[set].p;
     const double* d_dy = (const double*)ctx->h_dy[set].p;
     int64_t tf = 0, tb = 0;
-    ctx->last_row_ptr = nullptr;  // staging pointers are reused across sub-batches: never trust the cache
+    ctx->prep_valid = false;  // staging pointers are reused across sub-batches: the records are another sub-batch's
     rc = qlp_bls_grid(ctx, S, d_row, d_t, (const double*)ctx->h_rho[set].p, nullptr,
                       (qlp_bls_star_grid*)ctx->h_grid.p, (int64_t*)ctx->h_fptr.p, &tf, &tb, st);
     if (rc != 0) break;
@@ -642,7 +685,6 @@ static int search_host_impl(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* ro
   }
   // everything enqueued (or failed): drain both streams before the host buffers go out of scope
   cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(ctx->copy_stream);
-  free(row_tmp[0]); free(row_tmp[1]);
   if (rc == 0 && (e1 != cudaSuccess || e2 != cudaSuccess)) { cudaGetLastError(); rc = QLP_BLS_ECUDA; }
   if (rc == 0 && total_freq) *total_freq = tf_sum;
   return rc;
@@ -694,8 +736,8 @@ extern "C" int qlp_bls_debug_prep(qlp_bls_ctx* ctx, const int64_t* row_ptr, cons
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(ctx->device));
   // the prep kernel runs over the whole batch; the caller passes the batch size through the grid call
-  if (ctx->last_row_ptr != row_ptr || ctx->last_n_stars <= star) return QLP_BLS_EINVAL;
-  QLP_TRY(run_prep(ctx, ctx->last_n_stars, row_ptr, t, y, dy, grid, st));
+  if (ctx->grid_row_ptr != row_ptr || ctx->grid_n_stars <= star) return QLP_BLS_EINVAL;
+  QLP_TRY(run_prep(ctx, ctx->grid_n_stars, row_ptr, t, y, dy, grid, st));
   debug_prep_kernel<<<64, 256, 0, st>>>(row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, star, tau, w, wy);
   return launch_ok(ctx);
 }

@@ -153,7 +153,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const int64_t* __restrict__ tile_off, const int64_t* __restrict__ kb,
     unsigned long long* __restrict__ counter, float* __restrict__ sr, uint32_t* __restrict__ best,
-    unsigned long long* __restrict__ phase /* NULL, or 3 counters: set-up, fold, scan clocks of thread 0 */) {
+    unsigned long long* __restrict__ phase /* NULL, or this class's 5 counters: set-up, fold, scan clocks of
+                                              thread 0, point x frequency evaluations, tiles */) {
   extern __shared__ __align__(16) unsigned char smem[];
   Point* pbuf = reinterpret_cast<Point*>(smem);                          // [2][kChunk]
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem + 2 * kChunk * 16);  // [2]
@@ -418,7 +419,11 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         // take the narrowest ladder width that still covers the occupied span and, for it, the
         // smallest start bin whose extra bins are all empty.
         const uint32_t* hc = hist + scol;
-        auto empty = [&](int e) { e %= nbk; if (e < 0) e += nbk; return hc[e * STRIDE] == 0u; };
+        // a bin is empty only if both words are zero (a point of tiny weight may quantise to W = 0 with S != 0)
+        auto empty = [&](int e) {
+          e %= nbk; if (e < 0) e += nbk;
+          return (hc[e * STRIDE] | hc[e * STRIDE + CTOT]) == 0u;
+        };
         int a = bj, b = bj + bm - 1;
         while (a < b && empty(a)) ++a;
         while (b > a && empty(b)) --b;
@@ -448,6 +453,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       atomicAdd(&phase[0], (unsigned long long)(clk1s - clk0));
       atomicAdd(&phase[1], (unsigned long long)(clk2 - clk1s));
       atomicAdd(&phase[2], (unsigned long long)(clk3 - clk2));
+      atomicAdd(&phase[3], (unsigned long long)ti.n_pts * (unsigned long long)ti.ncols);
+      atomicAdd(&phase[4], 1ull);
     }
   }
 }

@@ -24,14 +24,20 @@ __global__ void __launch_bounds__(256) grid_kernel(Params prm, int64_t n_stars, 
   __shared__ int n_brk;
   __shared__ qlp_bls_star_grid g;
   __shared__ unsigned long long bins_acc;
-  if (threadIdx.x == 0) { n_brk = 0; bins_acc = 0ull; }
+  __shared__ int bad_t;
+  if (threadIdx.x == 0) { n_brk = 0; bins_acc = 0ull; bad_t = 0; }
   __syncthreads();
-  // O1.2: position i is a break if t[i+1] - t[i] > sector_days (strict).
+  // O1.2: position i is a break if t[i+1] - t[i] > sector_days (strict).  The same differences show whether
+  // the timestamps increase strictly (the contract of the API): a star that breaks it would fold with
+  // tau < 0, for which the fold's magic-number floor is not defined, so it is skipped here (status 7)
+  // whether or not input validation (flags bit0) is on.
   for (int64_t i = threadIdx.x; i + 1 < n; i += blockDim.x) {
-    if (dsub(ts[i + 1], ts[i]) > prm.sector_days) {
+    const double d = dsub(ts[i + 1], ts[i]);
+    if (d > prm.sector_days) {
       int slot = atomicAdd(&n_brk, 1);
       if (slot < kMaxBreaks) brk[slot] = i;
     }
+    if (!(d > 0.0) || !(d < 1.0e15)) bad_t = 1;   // repeated, decreasing, NaN or infinite timestamps
   }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -111,7 +117,8 @@ __global__ void __launch_bounds__(256) grid_kernel(Params prm, int64_t n_stars, 
           q.u0 = u0; q.h = h;
           double qlo = dmul(Q, dmul(u0, u0));
           q.nb_max = (int32_t)ceil(ddiv((double)prm.noverlap, qlo));
-          if (q.nb_max > QLP_BLS_MAX_NB || q.nb_max <= 0) { q.status = 4; q.n_freq = 0; }
+          if (bad_t) { q.status = 7; q.n_freq = 0; }
+          else if (q.nb_max > QLP_BLS_MAX_NB || q.nb_max <= 0) { q.status = 4; q.n_freq = 0; }
           else if (n >= (int64_t)QLP_BLS_MAX_POINTS) { q.status = 5; q.n_freq = 0; }  // fixed-point weights
         }
       }

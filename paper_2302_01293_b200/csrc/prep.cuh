@@ -10,8 +10,14 @@
 // histograms are integers:
 //   W_i = round(w_i * (2^32 - 2^22))        -> any sum of W_i stays below 2^32 for N < 2^23;
 //   S_i = round(w_i ytilde_i * scale_s)     -> scale_s chosen per star so that no phase bin of any
-//         grid frequency can overflow int32: a bin of duration <= Q/(noverlap u) holds at most
-//         floor(that / dt_min) + 1 points per cycle and is visited in at most f T + 2 cycles.
+//         grid frequency can overflow int32.  A bin of duration D <= Q/(noverlap u) is visited in at most
+//         C = f T + 2 cycles; for ANY spacing threshold d, a window of length D holds at most D/d + 1 points
+//         whose spacings are >= d, and every spacing below d adds at most one point to one window, so
+//             points per bin <= C (D/d + 1) + #{spacings < d}.
+//         The spacings are histogrammed in quarter-octave buckets and the best threshold is taken: a few
+//         near-coincident timestamps (overlapping sectors or cameras) cost a few counts, not the bound
+//         (with the plain minimum spacing one such pair would degrade the bound to N and cost
+//         log2(N / cnt) bits of S resolution on a long star).
 // One CTA per star, three passes over its points (the 2nd and 3rd hit L2).
 #pragma once
 #include "common.cuh"
@@ -47,6 +53,20 @@ __device__ __forceinline__ double block_max(double v, double* sh) {
   return sh[0];
 }
 
+// Quarter-octave buckets of the spacing between consecutive timestamps, 2^-40 d ... 2^12 d.  The bucket of d is
+// (biased exponent, top two mantissa bits) of its FP64 pattern; everything below 2^-40 d (zero, negative and NaN
+// spacings too) lands in bucket 0, everything above in the last one.
+constexpr int kSpLoExp = 1023 - 40;                    // biased exponent of 2^-40
+constexpr int kSpBuckets = 52 * 4;
+__device__ __forceinline__ int spacing_bucket(double d) {
+  if (!(d > 0.0)) return 0;
+  const int idx = (__double2hiint(d) >> 18) - (kSpLoExp << 2);
+  return idx < 0 ? 0 : (idx >= kSpBuckets ? kSpBuckets - 1 : idx);
+}
+__device__ __forceinline__ double spacing_bucket_edge(int b) {   // lower edge of bucket b
+  return __hiloint2double((b + (kSpLoExp << 2)) << 18, 0);
+}
+
 __global__ void __launch_bounds__(256) prep_kernel(Params prm, int64_t n_stars, const int64_t* __restrict__ row_ptr,
                                                    const double* __restrict__ t, const double* __restrict__ y,
                                                    const double* __restrict__ dy,
@@ -60,18 +80,20 @@ __global__ void __launch_bounds__(256) prep_kernel(Params prm, int64_t n_stars, 
   const double* ts = t + a;
   const double* ys = y + a;
   const double* ds = dy + a;
-  // pass 1: W_sum, sum y/dy^2, min spacing
-  double acc_w = 0.0, acc_wy = 0.0, dtmin = 1.0e300;
+  // pass 1: W_sum, sum y/dy^2, histogram of the spacings in quarter-octave buckets
+  __shared__ unsigned int sp_hist[kSpBuckets];
+  for (int i = threadIdx.x; i < kSpBuckets; i += blockDim.x) sp_hist[i] = 0u;
+  __syncthreads();
+  double acc_w = 0.0, acc_wy = 0.0;
   for (int64_t i = threadIdx.x; i < n; i += blockDim.x) {
     double d = ds[i];
     double iv = 1.0 / (d * d);
     acc_w += iv;
     acc_wy += iv * ys[i];
-    if (i + 1 < n) dtmin = fmin(dtmin, ts[i + 1] - ts[i]);
+    if (i + 1 < n) atomicAdd(&sp_hist[spacing_bucket(ts[i + 1] - ts[i])], 1u);
   }
   const double W = block_sum(acc_w, sh);
   const double WY = block_sum(acc_wy, sh);
-  const double dt_min = -block_max(-dtmin, sh);
   const double ybar = (n > 0) ? WY / W : 0.0;
   // pass 2: max |w ytilde|
   double mx = 0.0;
@@ -82,17 +104,33 @@ __global__ void __launch_bounds__(256) prep_kernel(Params prm, int64_t n_stars, 
   }
   const double wy_max = block_max(mx, sh);
   // bound on the number of points that can share one phase bin at any grid frequency
-  double cnt = (double)n;
-  if (g.status == 0 && g.n_freq > 0 && dt_min > 0.0) {
-    const double Q = prm.qmin_fac * g.c_q;
-    const double u_lo = g.u0, u_hi = g.u0 + (double)g.n_freq * g.h;
-    const double no = (double)prm.noverlap;
-    double b = Q * g.baseline * u_hi * u_hi / (no * dt_min) + 2.0 * Q / (no * u_lo * dt_min) +
-               u_hi * u_hi * u_hi * g.baseline + 2.0;
-    b = b * 1.01 + 2.0;
-    if (b < cnt) cnt = b;
+  // (thread 0 walks the buckets; the result goes through shared memory so that every thread holds the same bits)
+  __shared__ double cnt_sh;
+  if (threadIdx.x == 0) {
+    double cnt = (double)n;
+    if (g.status == 0 && g.n_freq > 0) {
+      const double Q = prm.qmin_fac * g.c_q;
+      const double u_lo = g.u0, u_hi = g.u0 + (double)g.n_freq * g.h;
+      const double no = (double)prm.noverlap;
+      // sum over cycles of D/d: D = Q/(no u) days per bin and cycle, C = f T + 2 cycles, evaluated at the grid
+      // ends (u_hi for the f T part, u_lo for the + 2 part); cycles = C at the highest frequency
+      const double span = Q * g.baseline * u_hi * u_hi / no + 2.0 * Q / (no * u_lo);
+      const double cycles = u_hi * u_hi * u_hi * g.baseline + 2.0;
+      double n_small = 0.0;   // spacings below the lower edge of bucket b
+      for (int b = 0; b < kSpBuckets; ++b) {
+        const double d = spacing_bucket_edge(b);
+        if (b > 0) {          // bucket 0 also holds zero / negative / NaN spacings: no threshold below it
+          const double bound = (span / d + cycles) * 1.01 + 2.0 + n_small;
+          if (bound < cnt) cnt = bound;
+        }
+        n_small += (double)sp_hist[b];
+      }
+    }
+    if (cnt < 1.0) cnt = 1.0;
+    cnt_sh = cnt;
   }
-  if (cnt < 1.0) cnt = 1.0;
+  __syncthreads();
+  const double cnt = cnt_sh;
   double scale_s = 0.0;
   if (wy_max > 0.0 && isfinite(wy_max)) scale_s = (2147483647.0 - cnt - 1.0) / (cnt * wy_max);
   int32_t status = (n >= (1 << 22)) ? 5 : 0;

@@ -104,21 +104,11 @@ def _log_uniform(rng, lo, hi):
     return math.exp(rng.uniform(math.log(lo), math.log(hi)))
 
 
-def make_star(config: int, star_id: int, seed: int = 0):
-    """One star of the given config -> (t, y, dy, rho, rstar, truth tuple)."""
+def _star_layout(config: int, star_id: int, seed: int = 0):
+    """The part of a star that does not depend on its flux: timestamps (after the quality-flag drops), density,
+    radius, white-noise level and the injection ranges.  Consumes the star's random stream up to and including
+    the drop mask, so that :func:`make_star` continues from the same state.  Configs 2-5 only."""
     rng = np.random.default_rng([seed, config, star_id])
-    truth = (0.0, 0.0, 0.0, 0.0)
-    if config == 1:
-        t = sector_times(0, 1800.0)
-        sigma = 1e-3
-        rho, rstar = 1.0, 1.0
-        dy = np.full(t.shape, sigma)
-        y = rng.standard_normal(t.size) * sigma
-        period, depth, duration = 3.7, 2e-3, 2.5 / 24.0
-        t0 = t[0] + rng.uniform(0.0, period)
-        _inject(t, y, period, t0, depth, duration)
-        return t, y, dy, rho, rstar, (period, t0, depth, duration)
-
     rho = math.exp(rng.normal(0.0, 0.5))
     rstar = math.exp(rng.normal(0.0, 0.3))
     sigma = _log_uniform(rng, 2e-4, 1e-2)
@@ -155,9 +145,36 @@ def make_star(config: int, star_id: int, seed: int = 0):
         drop = 0.02
     else:
         raise ValueError(f"unknown config {config}")
-
     if drop > 0.0:
         t = t[rng.random(t.size) >= drop]
+    return rng, t, rho, rstar, sigma, red_fac, (inj_frac, p_lo, p_hi, d_lo, d_hi)
+
+
+def star_times(config: int, star_id: int, seed: int = 0):
+    """Timestamps and density of one star without generating its flux -> (t, rho).  What a cost estimate needs
+    (points x frequencies, for sharding stars over GPUs) at a fraction of the cost of :func:`make_star`."""
+    if config == 1:
+        return sector_times(0, 1800.0), 1.0
+    _, t, rho, _, _, _, _ = _star_layout(config, star_id, seed)
+    return t, rho
+
+
+def make_star(config: int, star_id: int, seed: int = 0):
+    """One star of the given config -> (t, y, dy, rho, rstar, truth tuple)."""
+    truth = (0.0, 0.0, 0.0, 0.0)
+    if config == 1:
+        rng = np.random.default_rng([seed, config, star_id])
+        t = sector_times(0, 1800.0)
+        sigma = 1e-3
+        rho, rstar = 1.0, 1.0
+        dy = np.full(t.shape, sigma)
+        y = rng.standard_normal(t.size) * sigma
+        period, depth, duration = 3.7, 2e-3, 2.5 / 24.0
+        t0 = t[0] + rng.uniform(0.0, period)
+        _inject(t, y, period, t0, depth, duration)
+        return t, y, dy, rho, rstar, (period, t0, depth, duration)
+
+    rng, t, rho, rstar, sigma, red_fac, (inj_frac, p_lo, p_hi, d_lo, d_hi) = _star_layout(config, star_id, seed)
     n = t.size
     dy = sigma * np.exp(0.1 * rng.standard_normal(n))
     y = rng.standard_normal(n) * dy + _ar1(rng, n, 0.9, red_fac * sigma)

@@ -175,17 +175,15 @@ def _compare_sr(sr_g, best_g, sr_o, m_o, j_o, label):
 
 
 def _check_best_valid(orc, cfg, b, go, s, ks, m_g, j_g, sr_o, tol):
-    """Where (m, j) differs from the oracle's, the GPU's box must be as good within the tolerance."""
+    """Where (m, j) differs from the oracle's, the GPU's box must be as good within the tolerance: EVERY such
+    frequency is re-evaluated under the oracle's arithmetic (orc_box_values)."""
+    ks = np.asarray(ks, dtype=np.int64)
+    if ks.size == 0:
+        return
     t, y, dy = b.star(s)
-    tau, w, wy = orc.prep(t, y, dy, float(go[s]["t_ref"]))
-    for k in ks:
-        f, nb = orc.freqs(cfg, go[s], int(k), int(k) + 1)
-        val = orc.sr_one(tau, w, wy, float(f[0]), int(nb[0]), np.array([m_g[k]]))  # best over j at the GPU's m
-        bo = orc.bins(float(f[0]), int(nb[0]), tau)
-        sel = ((bo - j_g[k]) % int(nb[0])) < m_g[k]
-        r, sv = w[sel].sum(), wy[sel].sum()
-        v = sv * sv / (r * (1 - r)) if 0 < r < 1 else 0.0
-        assert abs(v - sr_o[k]) <= 2 * tol, (s, k, v, sr_o[k], val)
+    v = orc.box_values(cfg, go[s], t, y, dy, ks, m_g[ks], j_g[ks])
+    worst = np.abs(v - sr_o[ks])
+    assert worst.max() <= 2 * tol, (s, int(ks[np.argmax(worst)]), float(worst.max()), tol)
 
 
 @pytest.mark.parametrize("name,path", [("c1", 0), ("c1", 2), ("c1", 3), ("c1", 4), ("c1", 5), ("c1", 6), ("c1", 7),
@@ -221,7 +219,7 @@ def test_sr_parity_full(gpu, ctx, orc, cfg, batches, name, path):
         if so.size >= 2 and so[top[1]] - so[top[0]] > SR_RTOL * so[top[1]]:
             assert int(np.argmax(sr[a:e])) == int(top[1])
         bad = np.nonzero((m_g != ob["m"][a:e]) | (j_g != ob["j"][a:e]))[0]
-        _check_best_valid(orc, cfg, b, ob["grid"], s, bad[:20], m_g, j_g, so, SR_RTOL * so.max())
+        _check_best_valid(orc, cfg, b, ob["grid"], s, bad, m_g, j_g, so, SR_RTOL * so.max())
     print(f"{name} path={path}: worst |dSR|/peak = {worst:.2e}, (m,j) identical on {np.mean(agree):.4f}")
     assert np.mean(agree) > 0.98
 

@@ -1,0 +1,369 @@
+"""Parity at the sizes production takes (run with -m gpu on a B200), all through the C ABI against oracle/.
+
+  (a) tile classes 6, 7 and 8 at their NATIVE histogram sizes: hand-built 30-min stars of 20, 30 and 40 sectors with
+      one hole longer than a sector (P_max = the longest stretch) so that nb_max lands in (3360, 6720],
+      (6720, 13440] and (13440, 24576]; bins bit-exact, SR and (m, j) on frequencies sampled towards the low end;
+  (b) whole spectra on the samples SURVEY.md 8(d) / BASELINE.md fix: all 1,000 stars of config 2, 256 of config 3,
+      16 of config 4, and a 256-star cost-stratified subset of config 5 (whole spectra for the stars the oracle
+      finishes in seconds, 150 sampled frequencies for the heavy ones, one of them with > 10^5 frequencies);
+      EVERY frequency where the GPU's (m, j) differs from the oracle's has the GPU's box re-evaluated by the oracle;
+  (c) S4 (median-binned trend, MAD, Sturges N) at n_freq >= 7e4 and >= 5e5, fed the GPU's SR;
+  (e) the worst case of the S fixed-point scale: a 40-sector 200-s star (456,000 points) with near-coincident
+      timestamps 1e-6 d apart.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SR_RTOL = 1e-4  # of the per-star peak (BASELINE.json north_star)
+CAPS = [94, 208, 420, 840, 1680, 3360, 6720, 13440, 24576]  # largest nb of tile class 0..8
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2302_01293_b200 import build, bls
+    build.build()
+    return bls
+
+
+@pytest.fixture(scope="module")
+def ctx(gpu):
+    c = gpu.QlpBls(top_k=3)
+    yield c
+    c.close()
+
+
+def _search(gpu, ctx, b, want_snr=False):
+    dev = gpu.upload(b)
+    grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+    sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+    out = dict(dev=dev, grid_dev=grid, fp_dev=fp, tf=tf, sr_dev=sr, best_dev=best, grid=gpu.grid_to_numpy(grid),
+               sr=sr.cpu().numpy(), best=best.cpu().numpy().view(np.uint32), fp=fp.cpu().numpy())
+    if want_snr:
+        snr, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best)
+        out["snr"] = snr.cpu().numpy()
+        out["peaks"] = gpu.peaks_to_numpy(peaks, ctx.top_k)
+    return out
+
+
+def _oracle_grids(orc, cfg, b):
+    gs = np.zeros(b.n_stars, dtype=orc.GRID_DTYPE)
+    for s in range(b.n_stars):
+        gs[s] = orc.grid(cfg, b.star(s)[0], float(b.rho[s]))
+    return gs
+
+
+def _class_of(nb):
+    return int(np.searchsorted(CAPS, nb))
+
+
+def _check_sampled(orc, cfg, b, s, go, res, ks, peak=None):
+    """SR and (m, j) of star s at the grid indices ks against the oracle; -> (worst |dSR| / peak, share of equal (m, j))."""
+    t, y, dy = b.star(s)
+    a = int(res["fp"][s])
+    sr_o, m_o, j_o = orc.spectrum_samples(cfg, go, t, y, dy, ks)
+    sr_g = res["sr"][a + ks].astype(np.float64)
+    if peak is None:
+        peak = float(sr_o.max())
+    tol = SR_RTOL * peak
+    err = np.abs(sr_g - sr_o)
+    assert err.max() <= tol, (s, int(ks[np.argmax(err)]), float(err.max()), tol)
+    bg = res["best"][a + ks]
+    m_g, j_g = (bg >> 24).astype(np.int32), (bg & 0xFFFFFF).astype(np.int32)
+    bad = np.nonzero((m_g != m_o) | (j_g != j_o))[0]
+    if bad.size:  # a different box must be as good, under the oracle's arithmetic: every one of them is checked
+        v = orc.box_values(cfg, go, t, y, dy, ks[bad], m_g[bad], j_g[bad])
+        worst = np.abs(v - sr_o[bad]).max()
+        assert worst <= 2 * tol, (s, float(worst), tol)
+    return float(err.max() / peak) if peak > 0 else 0.0, 1.0 - bad.size / ks.size
+
+
+def _check_whole(orc, cfg, b, s, go, res, ob):
+    """Whole spectrum of star s against orc.batch output ob."""
+    t, y, dy = b.star(s)
+    a, e = int(res["fp"][s]), int(res["fp"][s + 1])
+    assert (a, e) == (int(ob["freq_ptr"][s]), int(ob["freq_ptr"][s + 1]))
+    if e == a:
+        return 0.0, 1.0
+    sr_o, m_o, j_o = ob["sr"][a:e], ob["m"][a:e], ob["j"][a:e]
+    peak = float(sr_o.max())
+    tol = SR_RTOL * peak
+    err = np.abs(res["sr"][a:e].astype(np.float64) - sr_o)
+    assert err.max() <= tol, (s, int(np.argmax(err)), float(err.max()), tol)
+    bg = res["best"][a:e]
+    m_g, j_g = (bg >> 24).astype(np.int32), (bg & 0xFFFFFF).astype(np.int32)
+    bad = np.nonzero((m_g != m_o) | (j_g != j_o))[0]
+    if bad.size:
+        v = orc.box_values(cfg, go, t, y, dy, bad, m_g[bad], j_g[bad])
+        worst = np.abs(v - sr_o[bad]).max()
+        assert worst <= 2 * tol, (s, float(worst), tol)
+    # argmax frequency identical wherever the top two oracle values differ by more than the tolerance
+    if sr_o.size >= 2:
+        top = np.argsort(sr_o)[-2:]
+        if sr_o[top[1]] - sr_o[top[0]] > tol:
+            assert int(np.argmax(res["sr"][a:e])) == int(top[1])
+    return float(err.max() / peak) if peak > 0 else 0.0, 1.0 - bad.size / (e - a)
+
+
+# ---------------------------------------------------------------------------------------------- (a)
+def _long_star(n_sectors, cadence_s, rng, hole=2):
+    """n_sectors contiguous sectors, a hole of `hole` sectors (> 27.4 d: a break), one more sector."""
+    from paper_2302_01293_b200 import synth
+    secs = list(range(n_sectors)) + [n_sectors + hole]
+    t = np.concatenate([synth.sector_times(s, cadence_s) for s in secs])
+    dy = 1e-3 * np.exp(0.1 * rng.standard_normal(t.size))
+    y = rng.standard_normal(t.size) * dy
+    return t, y, dy
+
+
+def _k_of_nb(cfg, go, nb):
+    """Grid index whose nb_k is close to nb (nb_k = ceil(noverlap / (Q u^2)), u = u0 + k h)."""
+    Q = cfg.qmin_fac * float(go["c_q"])
+    u = np.sqrt(cfg.noverlap / (Q * float(nb)))
+    return int(np.clip(round((u - float(go["u0"])) / float(go["h"])), 0, int(go["n_freq"]) - 1))
+
+
+@pytest.mark.parametrize("n_sectors,rho,want_class", [(20, 1.0, 6), (30, 3.0, 7), (40, 10.0, 8)])
+def test_native_wide_tile_classes(gpu, ctx, orc, cfg, n_sectors, rho, want_class):
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(100 + n_sectors)
+    t, y, dy = _long_star(n_sectors, 1800.0, rng)
+    # a box transit at a long period, so that the low-frequency end holds the peak
+    period, depth = 0.31 * (t[-1] - t[0]) / 3.0, 3e-3
+    y = y - depth * (np.mod(t - t[0] - 5.0, period) < 0.6)
+    short = synth.sector_times(0, 1800.0)
+    b = synth.from_arrays([(short, rng.standard_normal(short.size) * 1e-3, np.full(short.size, 1e-3)), (t, y, dy)],
+                          rho=np.array([1.0, rho]))
+    res = _search(gpu, ctx, b)
+    go = _oracle_grids(orc, cfg, b)
+    assert res["grid"].tobytes() == go.tobytes()
+    g = go[1]
+    nf, nb_max = int(g["n_freq"]), int(g["nb_max"])
+    assert g["p_max"] == t[n_sectors * short.size - 1] - t[0]          # P_max = the longest stretch (one break)
+    assert _class_of(nb_max) == want_class, (nb_max, want_class)
+    # frequencies: the first ones, the class boundaries (both sides), the middle of every class reached, and a
+    # sample weighted to the low-frequency end
+    ks = {0, 1, 2, 3, nf - 1, nf // 2}
+    for c in range(0, want_class + 1):
+        lo = CAPS[c - 1] if c > 0 else 38
+        hi = min(CAPS[c], nb_max)
+        for nb in (hi, (lo + hi) // 2, lo + 1):
+            k = _k_of_nb(cfg, g, nb)
+            ks.update({k, min(k + 1, nf - 1), max(k - 1, 0)})
+    ks.update((rng.random(60) ** 3 * nf).astype(np.int64).tolist())
+    ks.update(rng.integers(0, nf, 20).tolist())
+    ks = np.array(sorted(ks), dtype=np.int64)
+    f_all, nb_all = orc.freqs(cfg, g, 0, nf)
+    reached = {_class_of(int(nb_all[k])) for k in ks}
+    assert reached == set(range(0, want_class + 1)), reached
+    # O3: bin indices bit-exact (same device function as the fold) at the widest histograms
+    tau = t - g["t_ref"]
+    for k in ks[:6]:
+        bo = orc.bins(float(f_all[k]), int(nb_all[k]), tau)
+        bg = ctx.debug_bins(res["dev"][0], res["dev"][1], res["grid_dev"], 1, int(k), t.size).cpu().numpy()
+        assert np.array_equal(bg, bo), (int(k), int((bg != bo).sum()))
+    worst, same = _check_sampled(orc, cfg, b, 1, g, res, ks)
+    # whole spectrum of the short neighbour (tiles of both stars share the persistent CTAs)
+    ob = orc.batch(cfg, b.row_ptr[:2], b.t[:short.size], b.y[:short.size], b.dy[:short.size], b.rho[:1], K=0,
+                   want_snr=False)
+    _check_whole(orc, cfg, b, 0, go[0], res, ob)
+    print(f"class {want_class}: nb_max={nb_max}, n_freq={nf}, {ks.size} sampled frequencies, worst |dSR|/peak="
+          f"{worst:.2e}, (m,j) identical on {same:.3f}")
+    assert same > 0.9
+
+
+# ---------------------------------------------------------------------------------------------- (b)
+@pytest.mark.parametrize("config,n_stars", [(2, 1000), (3, 256), (4, 16)])
+def test_whole_spectrum_parity_contract_samples(gpu, ctx, orc, cfg, config, n_stars):
+    """SURVEY.md 8(d) "parity checks run on exactly these stars": all of config 2, 256 stars of config 3, 16 of
+    config 4 -- every frequency of every star, element by element (the oracle runs OpenMP over the stars)."""
+    from paper_2302_01293_b200 import synth
+    b = synth.make_batch(config, n_stars=n_stars)
+    res = _search(gpu, ctx, b)
+    ob = orc.batch(cfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=0, want_snr=False)
+    assert res["grid"].tobytes() == ob["grid"].tobytes()
+    assert np.array_equal(res["fp"], ob["freq_ptr"])
+    worst, same = 0.0, []
+    for s in range(b.n_stars):
+        w, sm = _check_whole(orc, cfg, b, s, ob["grid"][s], res, ob)
+        worst = max(worst, w)
+        same.append(sm)
+    print(f"config {config}: {n_stars} stars, {int(res['tf'])} frequencies, worst |dSR|/peak = {worst:.2e}, "
+          f"(m,j) identical on {np.mean(same):.4f} (min over stars {np.min(same):.4f})")
+    assert np.mean(same) > 0.98
+
+
+def test_whole_spectrum_parity_config5_stratified(gpu, ctx, orc, cfg):
+    """256 stars of config 5 (BASELINE.json configs[4]) taken at evenly spaced ranks of the cost N_pts x n_freq of
+    its first 2,000 stars (so the heaviest and the lightest are in).  Stars the oracle finishes in seconds are
+    compared on whole spectra; the heavy ones (more than 3e9 evaluations) on 150 frequencies each, weighted to the
+    low-frequency (large nb) end, plus the GPU's own peak frequency."""
+    from paper_2302_01293_b200 import synth
+    n_pool = 2000
+    cost = np.zeros(n_pool)
+    for sid in range(n_pool):
+        t, _, _, rho, _, _ = synth.make_star(5, sid)
+        cost[sid] = float(orc.grid(cfg, t, rho)["n_freq"]) * t.size
+    order = np.argsort(cost, kind="stable")
+    ids = np.unique(order[np.linspace(0, n_pool - 1, 256).round().astype(np.int64)])
+    b = synth.make_batch(5, star_ids=ids)
+    res = _search(gpu, ctx, b)
+    go = _oracle_grids(orc, cfg, b)
+    assert res["grid"].tobytes() == go.tobytes()
+    assert go["n_freq"].max() > 100000
+    c = cost[ids]
+    light = np.nonzero(c <= 3e9)[0]
+    heavy = np.nonzero(c > 3e9)[0]
+    assert light.size > 150 and heavy.size >= 10
+    # whole spectra of the light stars, one oracle batch
+    bl = synth.make_batch(5, star_ids=ids[light])
+    ob = orc.batch(cfg, bl.row_ptr, bl.t, bl.y, bl.dy, bl.rho, K=0, want_snr=False)
+    worst, same = 0.0, []
+    for i, s in enumerate(light):
+        a, e = int(res["fp"][s]), int(res["fp"][s + 1])
+        ao, eo = int(ob["freq_ptr"][i]), int(ob["freq_ptr"][i + 1])
+        assert e - a == eo - ao
+        if e == a:
+            continue
+        t, y, dy = b.star(int(s))
+        sr_o, m_o, j_o = ob["sr"][ao:eo], ob["m"][ao:eo], ob["j"][ao:eo]
+        peak = float(sr_o.max())
+        tol = SR_RTOL * peak
+        err = np.abs(res["sr"][a:e].astype(np.float64) - sr_o)
+        assert err.max() <= tol, (int(ids[s]), int(np.argmax(err)), float(err.max()), tol)
+        bg = res["best"][a:e]
+        m_g, j_g = (bg >> 24).astype(np.int32), (bg & 0xFFFFFF).astype(np.int32)
+        bad = np.nonzero((m_g != m_o) | (j_g != j_o))[0]
+        if bad.size:
+            v = orc.box_values(cfg, go[s], t, y, dy, bad, m_g[bad], j_g[bad])
+            assert np.abs(v - sr_o[bad]).max() <= 2 * tol, int(ids[s])
+        worst = max(worst, float(err.max() / peak))
+        same.append(1.0 - bad.size / (e - a))
+    # sampled frequencies of the heavy stars
+    rng = np.random.default_rng(55)
+    for s in heavy:
+        nf = int(go[s]["n_freq"])
+        a = int(res["fp"][s])
+        k_peak = int(np.argmax(res["sr"][a:a + nf]))
+        ks = np.unique(np.concatenate([[0, 1, 2, nf - 1, k_peak], (rng.random(100) ** 3 * nf).astype(np.int64),
+                                       rng.integers(0, nf, 45)]))
+        # the tolerance is relative to the star's peak: the sample holds the GPU's peak frequency, and the peak the
+        # oracle finds there is at most the true one, which makes the check stricter, never looser
+        w, sm = _check_sampled(orc, cfg, b, int(s), go[s], res, ks)
+        worst = max(worst, w)
+        same.append(sm)
+    print(f"config 5: {light.size} whole spectra + {heavy.size} sampled stars (n_freq up to {int(go['n_freq'].max())}, "
+          f"nb_max up to {int(go['nb_max'].max())}), worst |dSR|/peak = {worst:.2e}, (m,j) identical on "
+          f"{np.mean(same):.4f}")
+    assert np.mean(same) > 0.98
+
+
+# ---------------------------------------------------------------------------------------------- (c)
+def _check_snr_given_gpu_sr(gpu, ctx, orc, cfg, b, res, go, stars):
+    """S/N and peaks of the S4 kernel against orc.snr / orc.peak_indices fed the GPU's own SR."""
+    worst = 0.0
+    for s in stars:
+        a, e = int(res["fp"][s]), int(res["fp"][s + 1])
+        f, _ = orc.freqs(cfg, go[s])
+        sr64 = res["sr"][a:e].astype(np.float64)
+        sn_o, _, sigma = orc.snr(f, sr64)
+        scale = float(np.abs(sn_o).max())
+        d = float(np.abs(res["snr"][a:e] - sn_o).max())
+        assert d <= 1e-5 * scale + 1e-6, (s, e - a, d, scale)
+        worst = max(worst, d / scale)
+        idx = orc.peak_indices(sn_o, ctx.top_k)
+        vals = sn_o[idx]
+        pk = res["peaks"][s]
+        for r, k in enumerate(idx):
+            # ranks are unique only where no other local maximum is within the tolerance of this one
+            lm = np.nonzero((sn_o[1:-1] > sn_o[:-2]) & (sn_o[1:-1] >= sn_o[2:]))[0] + 1
+            close = lm[np.abs(sn_o[lm] - vals[r]) <= 1e-4 * scale]
+            if np.any(close != k):
+                continue
+            assert pk[r]["k"] == k, (s, r, pk["k"], idx)
+            assert abs(pk[r]["snr"] - sn_o[k]) <= 1e-5 * scale + 1e-6
+            assert pk[r]["nb"] == orc.freqs(cfg, go[s], int(k), int(k) + 1)[1][0] and pk[r]["freq"] == f[k]
+    return worst
+
+
+def test_snr_at_production_grid_sizes(gpu, ctx, orc, cfg):
+    """Config 4 (7e4-1.3e5 frequencies, Sturges N = 17-18) and the longest config-5 star of the first 2,000
+    (> 5e5 frequencies, N = 20-21: radix select over megabytes of SR, several thousand values per thread)."""
+    from paper_2302_01293_b200 import synth
+    b4 = synth.make_batch(4, n_stars=3)
+    res = _search(gpu, ctx, b4, want_snr=True)
+    go = _oracle_grids(orc, cfg, b4)
+    assert go["n_freq"].min() >= 50000
+    w4 = _check_snr_given_gpu_sr(gpu, ctx, orc, cfg, b4, res, go, range(b4.n_stars))
+    nf_best, sid_best = 0, -1
+    for sid in range(2000):
+        t, _, _, rho, _, _ = synth.make_star(5, sid)
+        if t.size < 30000:
+            continue
+        nf = int(orc.grid(cfg, t, rho)["n_freq"])
+        if nf > nf_best:
+            nf_best, sid_best = nf, sid
+    assert nf_best >= 500000
+    b5 = synth.make_batch(5, star_ids=np.array([0, sid_best, 3]))   # the long star between two ordinary ones
+    res = _search(gpu, ctx, b5, want_snr=True)
+    go = _oracle_grids(orc, cfg, b5)
+    assert orc.sturges(nf_best) >= 20
+    w5 = _check_snr_given_gpu_sr(gpu, ctx, orc, cfg, b5, res, go, range(b5.n_stars))
+    print(f"S4: config 4 n_freq {go['n_freq'].tolist()} worst {w4:.2e}; config 5 star {sid_best} n_freq {nf_best} "
+          f"(Sturges N = {orc.sturges(nf_best)}) worst {w5:.2e} of max|S/N|")
+
+
+# ---------------------------------------------------------------------------------------------- (e)
+def test_s_scale_with_near_coincident_timestamps(gpu, ctx, orc, cfg):
+    """40 sectors at 200 s (456,000 points) with a few timestamp pairs 1e-6 d apart (overlapping sectors or
+    cameras): the fixed-point scale of S must not collapse to the all-points-in-one-bin bound (prep.cuh)."""
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(77)
+    t = np.concatenate([synth.sector_times(s, 200.0) for s in range(40)])
+    extra = t[rng.integers(1000, t.size - 1000, 5)] + 1e-6
+    t = np.sort(np.concatenate([t, extra]))
+    assert np.diff(t).min() < 2e-6 and np.all(np.diff(t) > 0)
+    dy = 1e-3 * np.exp(0.1 * rng.standard_normal(t.size))
+    y = rng.standard_normal(t.size) * dy
+    y -= 2e-4 * (np.mod(t - t[0] - 3.0, 11.3) < 0.2)
+    b = synth.from_arrays([(t, y, dy)])
+    res = _search(gpu, ctx, b)
+    go = _oracle_grids(orc, cfg, b)
+    assert res["grid"].tobytes() == go.tobytes()
+    nf = int(go[0]["n_freq"])
+    k_peak = int(np.argmax(res["sr"][:nf]))
+    ks = np.unique(np.concatenate([[0, 1, nf - 1, k_peak], (rng.random(40) ** 3 * nf).astype(np.int64),
+                                   rng.integers(0, nf, 20)]))
+    worst, same = _check_sampled(orc, cfg, b, 0, go[0], res, ks)
+    print(f"S-scale worst case: {t.size} points, n_freq={nf}, worst |dSR|/peak = {worst:.2e}")
+    assert worst <= 2e-5       # quantisation stays far inside the 1e-4 tolerance
+
+
+def test_non_increasing_timestamps_are_contained(gpu, orc, cfg):
+    """A star whose timestamps repeat or go backwards is skipped (status 7) whether or not validation is on; its
+    neighbours are searched as usual."""
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(8)
+    t = synth.sector_times(0, 1800.0)
+    mk = lambda tt: (tt, rng.standard_normal(tt.size) * 1e-3, np.full(tt.size, 1e-3))
+    t_rep = t.copy(); t_rep[200] = t_rep[199]
+    t_back = t.copy(); t_back[300:] -= 5.0
+    t_nan = t.copy(); t_nan[17] = np.nan
+    b = synth.from_arrays([mk(t), mk(t_rep), mk(t_back), mk(t_nan), mk(t)])
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        res = _search(gpu, ctx, b, want_snr=True)
+        assert res["grid"]["status"].tolist() == [0, 7, 7, 7, 0]
+        assert res["grid"]["n_freq"][1:4].tolist() == [0, 0, 0]
+        assert np.all(res["peaks"][1:4]["k"] == -1)
+        go = orc.grid(cfg, t, 1.0)
+        for s in (0, 4):
+            so, _, _ = orc.spectrum_star(cfg, go, *b.star(s))
+            a, e = int(res["fp"][s]), int(res["fp"][s + 1])
+            assert np.abs(res["sr"][a:e] - so).max() <= SR_RTOL * so.max()
+    finally:
+        ctx.close()

@@ -212,3 +212,35 @@ def test_injection_recovery_config1(orc, cfg):
     # noiseless expectation delta^2 r (1-r) with r ~ duration/period
     r = tr["duration"] / tr["period"]
     assert 0.5 < pk["sr"] / (tr["depth"] ** 2 * r * (1 - r)) < 2.0
+
+
+# ------------------------------------------------------------------ test helpers of the oracle
+def test_sampled_spectrum_and_box_values_helpers(orc, cfg):
+    """orc_spectrum_samples is orc_spectrum_star restricted to some k (bitwise); orc_box_values agrees with a numpy
+    evaluation of the same box written here from the definition (weights, bins from exact rationals' floor)."""
+    b = synth.make_batch(2, n_stars=1)
+    t, y, dy = b.star(0)
+    t, y, dy = t[::8], y[::8], dy[::8]
+    g = orc.grid(cfg, t, float(b.rho[0]))
+    sr, m, j = orc.spectrum_star(cfg, g, t, y, dy)
+    rng = np.random.default_rng(5)
+    ks = np.unique(np.concatenate([[0, int(g["n_freq"]) - 1], rng.integers(0, int(g["n_freq"]), 40)]))
+    s2, m2, j2 = orc.spectrum_samples(cfg, g, t, y, dy, ks)
+    assert np.array_equal(s2, sr[ks]) and np.array_equal(m2, m[ks]) and np.array_equal(j2, j[ks])
+    # the best box re-evaluated point by point reproduces SR (summation order differs: 1e-12)
+    v = orc.box_values(cfg, g, t, y, dy, ks, m[ks], j[ks])
+    assert np.abs(v - sr[ks]).max() <= 1e-12 * sr.max()
+    # an arbitrary other box, from the definition in numpy
+    w = dy ** -2.0 / np.sum(dy ** -2.0)
+    yt = y - np.sum(w * y)
+    for k in ks[:10]:
+        (f,), (nb,) = orc.freqs(cfg, g, int(k), int(k) + 1)
+        mm, jj = int(rng.integers(3, 12)), int(rng.integers(0, nb))
+        ph = np.array([float(Fraction(float(f) * float(x)) % 1) for x in (t - t[0])])
+        bins = np.floor(ph * nb).astype(np.int64)
+        sel = ((bins - jj) % nb) < mm
+        r, s = w[sel].sum(), (w * yt)[sel].sum()
+        want = s * s / (r * (1 - r)) if 0 < r < 1 else 0.0
+        got = orc.box_values(cfg, g, t, y, dy, [k], [mm], [jj])[0]
+        assert abs(got - want) <= 1e-9 * max(want, 1e-30)
+        assert got <= sr[k] * (1 + 1e-12)      # no box beats the maximum
