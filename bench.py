@@ -52,7 +52,10 @@ N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum over the foldscan launches of ONE step of a named workload, from an
 # `ncu --set full` capture kept under profiles/ (not measured in this run: a run under ncu is never a bench value).
 NCU_TRAFFIC = {
-    (2, 1000): (719.3e6, "profiles/r1_foldscan_ncu.txt"),
+    (5, 4000): (7.831e9, "profiles/r2_launches.md (ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum over the "
+                         "nine foldscan launches of one step of this workload)"),
+    (2, 1000): (719.3e6, "profiles/r1_foldscan_ncu.txt (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum "
+                         "over the foldscan launches of one step)"),
 }
 CLASS_COLS = [128, 128, 64, 32, 16, 8, 4, 2, 1]
 CLASS_NBCAP = [94, 208, 420, 840, 1680, 3360, 6720, 13440, 24576]
@@ -557,8 +560,7 @@ def run_gpu(args):
                      # measured DRAM bytes of the foldscan launches of one step, from an ncu capture of THIS workload
                      # kept under profiles/ (null if there is none), next to the method's compulsory bytes
                      "traffic": traffic[0] if traffic else None,
-                     "traffic_source": (traffic[1] + " (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum "
-                                        "over the foldscan launches of one step; not measured in this run)")
+                     "traffic_source": (traffic[1] + "; a constant from that capture, not measured in this run")
                                        if traffic else None,
                      "compulsory_bytes_per_step": 16 * n_points + 8 * n_freq,
                      "compulsory_bytes_note": "16 B per point record read once + 8 B per frequency (SR + best) written",

@@ -566,9 +566,20 @@ int orc_sizeof_peak_stats(void) { return (int)sizeof(orc_peak_stats); }
  *              linearly); chi2 = sum w (y - model)^2 with that solution.  If the weighted variance of sh is
  *              below 1e-9 (no point, or every point, at one level) delta = 0, z = weighted mean.
  *   search   : compass search over (c, q, q_in) from (0, q0, 0.25) with steps (D0/4, q0/4, 0.125), bounds
- *              c in [-D0, D0], q in [0, 1], q_in in [0, 0.5]: sweep the six moves (+,- per coordinate, in
- *              that order), accept a move iff chi2 strictly decreases; when a sweep accepts nothing halve the
- *              steps; 24 halvings; no sweep starts once 600 evaluations are spent (so at most 605).
+ *              c in [-D0, D0], q in [0, 1], q_in in [0, 0.5].  One sweep evaluates chi2 at the (up to) six
+ *              neighbours theta +- h_d e_d (order c+, c-, q+, q-, q_in+, q_in-; clipped to the bounds, skipped
+ *              if the clipped value is the current one), takes the FIRST neighbour in that order whose chi2 is
+ *              within tol of the smallest of them, and moves there iff it lowers chi2 by more than tol; a sweep
+ *              that does not move halves the steps; 24 halvings; no sweep starts once 1200 evaluations are
+ *              spent (so at most 1205).  tol = max(1e-9 chi2_best, 1e-12 G), chi2_best the current value and
+ *              G = sum w (y - ybar)^2 over the window.  chi2 values of two implementations differ by ~1e-15 G
+ *              (FP64 sums of ~10^3..10^5 terms in different orders), a million times less than tol on real data
+ *              (chi2 ~ G), so neither the choice of the neighbour nor the acceptance depends on the order in
+ *              which the points are added up -- except when a difference lands within that noise of tol itself,
+ *              about once in 10^6 fits (once in 10^3 on noise-free data, where chi2 -> 0 and the 1e-12 G floor
+ *              is what stops the search).  (Reading changed in round 2: the first rule, "try the six moves in
+ *              turn, accept iff chi2 strictly decreases", was decided by rounding noise wherever chi2 is flat;
+ *              PAPER.md:44 names no optimiser.)
  * FP64; the sums run over the selected points in time order. */
 typedef struct {
   double t0, depth, q, q_in, z, chi2, chi2_init;
@@ -646,24 +657,35 @@ void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double
   double best = orc_trap_chi2(&fd, th[0], th[1], th[2], &dl, &z);
   int n_eval = 1;
   out->chi2_init = best;
-  for (int level = 0; level < 24 && n_eval < 600; ++level) {
+  const double tol_floor = 1e-12 * fd.G;
+  for (int level = 0; level < 24 && n_eval < 1200; ++level) {
     int moved = 1;
-    while (moved && n_eval < 600) {
+    while (moved && n_eval < 1200) {
       moved = 0;
-      for (int d = 0; d < 3; ++d) {
-        for (int sg = 0; sg < 2; ++sg) {
-          double c[3] = {th[0], th[1], th[2]};
-          double v = sg == 0 ? th[d] + h[d] : th[d] - h[d];
-          if (v < lo[d]) v = lo[d];
-          if (v > hi[d]) v = hi[d];
-          if (v == th[d]) continue;
-          c[d] = v;
-          double dl2, z2;
-          double chi = orc_trap_chi2(&fd, c[0], c[1], c[2], &dl2, &z2);
-          ++n_eval;
-          if (chi < best) { best = chi; th[d] = v; dl = dl2; z = z2; moved = 1; }
-        }
+      double tol = 1e-9 * best;
+      if (tol < tol_floor) tol = tol_floor;
+      double chi[6], dlk[6], zk[6], vk[6];
+      int have[6];
+      double cmin = 0.0;
+      int any = 0;
+      for (int k = 0; k < 6; ++k) {          /* k = 2 d + sg: c+, c-, q+, q-, q_in+, q_in- */
+        int d = k >> 1, sg = k & 1;
+        double c[3] = {th[0], th[1], th[2]};
+        double v = sg == 0 ? th[d] + h[d] : th[d] - h[d];
+        if (v < lo[d]) v = lo[d];
+        if (v > hi[d]) v = hi[d];
+        have[k] = (v != th[d]);
+        if (!have[k]) continue;
+        c[d] = v; vk[k] = v;
+        chi[k] = orc_trap_chi2(&fd, c[0], c[1], c[2], &dlk[k], &zk[k]);
+        ++n_eval;
+        if (!any || chi[k] < cmin) cmin = chi[k];
+        any = 1;
       }
+      if (!any) break;
+      int sel = -1;
+      for (int k = 0; k < 6 && sel < 0; ++k) if (have[k] && chi[k] <= cmin + tol) sel = k;
+      if (chi[sel] < best - tol) { best = chi[sel]; th[sel >> 1] = vk[sel]; dl = dlk[sel]; z = zk[sel]; moved = 1; }
     }
     h[0] *= 0.5; h[1] *= 0.5; h[2] *= 0.5;
   }

@@ -48,7 +48,7 @@ struct qlp_bls_ctx {
   int32_t force_path = 0;
   int64_t launches = 0;
   // workspace
-  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work, class_ctr;
+  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work, fit_chunk, fit_list, class_ctr;
   // host-API staging
   DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats, h_fits, h_pink;
   static const int kSide = 3;           // side streams for the independent tile-class launches
@@ -58,7 +58,7 @@ struct qlp_bls_ctx {
   cudaStream_t copy_stream = nullptr;  // H2D of the next sub-batch overlaps the search of the current one
   cudaEvent_t h2d_done[2], set_free[2];
   bool copy_ready = false;
-  int64_t* totals_host = nullptr;  // pinned, 4 x int64
+  int64_t* totals_host = nullptr;  // pinned, 8 x int64
   // The prepared point records (S0) in `pts` / `prep` belong to the arrays of the last run_prep call; qlp_bls_snr
   // reuses them only if it is given the same arrays and nothing else wrote the workspace since.
   struct PrepKey {
@@ -174,14 +174,16 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
                                  smem_for_cols(CT_)) == cudaSuccess &&                                               \
             cudaFuncSetAttribute(foldscan_kernel<16, CT_, 0u>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
                                  smem_for_cols(CT_)) == cudaSuccess
-  attr_ok = attr_ok && cudaFuncSetAttribute(fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            kFitSmemBytes) == cudaSuccess;
+  attr_ok = attr_ok &&
+            cudaFuncSetAttribute(fit_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kFitSmemBytes) == cudaSuccess &&
+            cudaFuncSetAttribute(fit_kernel<kFitCluster>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 kFitSmemBytes) == cudaSuccess;
   QLP_ATTR(128); QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
   if (!attr_ok ||
       cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
   }
-  if (cudaMallocHost((void**)&ctx->totals_host, 4 * sizeof(int64_t)) != cudaSuccess) {
+  if (cudaMallocHost((void**)&ctx->totals_host, 8 * sizeof(int64_t)) != cudaSuccess) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ENOMEM;
   }
   if (ctx->totals_dev.ensure(8 * sizeof(int64_t)) != 0) { cudaFreeHost(ctx->totals_host); delete ctx; return QLP_BLS_ENOMEM; }
@@ -193,7 +195,7 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   if (!ctx) return QLP_BLS_OK;
   cudaSetDevice(ctx->device);
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
-                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->class_ctr, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
+                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->fit_chunk, &ctx->fit_list, &ctx->class_ctr, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
                     &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats, &ctx->h_fits, &ctx->h_pink};
   for (DevBuf* b : bufs) b->release();
@@ -365,6 +367,18 @@ static int run_prep(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, c
   return 0;
 }
 
+// side streams for launches that are independent of one another (tile classes; large and small fits)
+static int ensure_side_streams(qlp_bls_ctx* ctx) {
+  if (ctx->fork_ready) return 0;
+  for (int i = 0; i < qlp_bls_ctx::kSide; ++i) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&ctx->side_done[i], cudaEventDisableTiming));
+  }
+  CUDA_TRY(cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming));
+  ctx->fork_ready = true;
+  return 0;
+}
+
 // ---- S0 + S2 + S3 ---------------------------------------------------------------------------------
 extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                 const double* y, const double* dy, const qlp_bls_star_grid* grid,
@@ -396,14 +410,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
   if (ctx->timing) CUDA_TRY(cudaEventRecord(ctx->ev0[slot], st));
   // The class kernels are independent: they go to side streams so that the CTAs of the next class fill the SMs
   // that the tail of the previous one leaves idle (each launch is persistent: any number of resident CTAs works).
-  if (!ctx->fork_ready) {
-    for (int i = 0; i < qlp_bls_ctx::kSide; ++i) {
-      CUDA_TRY(cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
-      CUDA_TRY(cudaEventCreateWithFlags(&ctx->side_done[i], cudaEventDisableTiming));
-    }
-    CUDA_TRY(cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming));
-    ctx->fork_ready = true;
-  }
+  QLP_TRY(ensure_side_streams(ctx));
   CUDA_TRY(cudaEventRecord(ctx->fork_ev, st));
   for (int i = 0; i < qlp_bls_ctx::kSide; ++i) CUDA_TRY(cudaStreamWaitEvent(ctx->side[i], ctx->fork_ev, 0));
   cudaStream_t user_st = st;
@@ -489,26 +496,61 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
   CUDA_TRY(cudaSetDevice(ctx->device));
   int rc = ctx->fit_cnt.ensure((size_t)n_items * sizeof(int64_t));
   if (rc == 0) rc = ctx->fit_off.ensure((size_t)(n_items + 2) * sizeof(int64_t));
+  if (rc == 0) rc = ctx->fit_chunk.ensure((size_t)n_items * kFitCluster * sizeof(int32_t));
+  if (rc == 0) rc = ctx->fit_list.ensure((size_t)n_items * 2 * sizeof(int32_t) + 16);
   if (rc != 0) return rc;
   int64_t* cnt = (int64_t*)ctx->fit_cnt.p;
   int64_t* off = (int64_t*)ctx->fit_off.p;
+  int32_t* chunk = (int32_t*)ctx->fit_chunk.p;
+  int32_t* list = (int32_t*)ctx->fit_list.p;
+  // two counters (items per size class) behind the lists, 8-byte aligned
+  unsigned long long* list_n = (unsigned long long*)((char*)ctx->fit_list.p + (((size_t)n_items * 2 * sizeof(int32_t) + 7) & ~(size_t)7));
+  CUDA_TRY(cudaMemsetAsync(list_n, 0, 16, st));
   const unsigned n_cta = (unsigned)((n_items + kFitWarps - 1) / kFitWarps);
-  fit_count_kernel<<<n_cta, kFitWarps * 32, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, peaks, cnt);
+  fit_count_kernel<<<n_cta, kFitWarps * 32, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, peaks, cnt, chunk, list, list_n);
   rc = launch_ok(ctx);
   if (rc != 0) return rc;
   fit_scan_kernel<<<1, 1024, 0, st>>>(n_items, cnt, off, off + n_items + 1);
   rc = launch_ok(ctx);
   if (rc != 0) return rc;
   CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 2, off + n_items, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(ctx->totals_host + 4, list_n, 16, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   const int64_t total = ctx->totals_host[2];
-  if (total < 0) return QLP_BLS_ECUDA;
+  const int64_t n_single = ctx->totals_host[4], n_cluster = ctx->totals_host[5];
+  if (total < 0 || n_single < 0 || n_cluster < 0 || n_single + n_cluster != n_items) return QLP_BLS_ECUDA;
   // a single window never holds more points than its star, and a star is capped at QLP_BLS_MAX_POINTS < 2^31
   rc = ctx->fit_work.ensure((size_t)(total > 0 ? total : 1) * 3 * sizeof(double));
   if (rc != 0) return rc;
-  fit_kernel<<<(unsigned)n_items, kFitThreads, kFitSmemBytes, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks, off,
-                                                (double*)ctx->fit_work.p, fits);
-  return launch_ok(ctx);
+  // Large windows first, on a side stream: one cluster of kFitCluster CTAs per item; the single-CTA fits of the small
+  // windows run beside them on the caller's stream.  Both grids are exact (the size classes were counted above).
+  QLP_TRY(ensure_side_streams(ctx));
+  CUDA_TRY(cudaEventRecord(ctx->fork_ev, st));
+  CUDA_TRY(cudaStreamWaitEvent(ctx->side[0], ctx->fork_ev, 0));
+  if (n_cluster > 0) {
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)(n_cluster * kFitCluster));
+    lc.blockDim = dim3(kFitThreads);
+    lc.dynamicSmemBytes = kFitSmemBytes;
+    lc.stream = ctx->side[0];
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = kFitCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&lc, fit_kernel<kFitCluster>, n_items, (int)ctx->prm.top_k, row_ptr, t, y, dy, peaks,
+                                (const int64_t*)off, (const int32_t*)chunk, (const int32_t*)(list + n_items), n_cluster,
+                                (double*)ctx->fit_work.p, fits));
+    QLP_TRY(launch_ok(ctx));
+  }
+  if (n_single > 0) {
+    fit_kernel<1><<<(unsigned)n_single, kFitThreads, kFitSmemBytes, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks,
+                                                                        off, chunk, list, n_single,
+                                                                        (double*)ctx->fit_work.p, fits);
+    QLP_TRY(launch_ok(ctx));
+  }
+  CUDA_TRY(cudaEventRecord(ctx->side_done[0], ctx->side[0]));
+  CUDA_TRY(cudaStreamWaitEvent(st, ctx->side_done[0], 0));
+  return QLP_BLS_OK;
 }
 
 // ---- O9: noise estimates, S/N_pink, detection criteria ------------------------------------------------

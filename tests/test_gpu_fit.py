@@ -1,13 +1,12 @@
 """O8 parity on the GPU: trapezoid fit of every peak against the oracle, through the C ABI.
 
 Both sides run the same compass search in FP64 on the same points.  The window membership is an integer decision
-taken with the same unfused operations (n_fit: bit-exact).  The trial parameters are sums and halvings of the same
-numbers, so the two paths are identical unless a chi2 comparison falls inside the rounding noise of two summation
-orders (relative 1e-13), which happens on noise peaks whose chi2 is flat along some direction (measured: about one
-fit in twelve, parameters then differ by up to 4e-5 relative at equal chi2).  So the test compares what is unique --
-the minimum reached (1e-8 relative) -- checks that the GPU's parameters are valid by evaluating the ORACLE's chi2,
-depth and level at them (1e-9 / 1e-6), bounds the parameter differences (1e-3), and demands that at least 70 % of the
-fits end at the same point (1e-9) after the same number of evaluations."""
+taken with the same unfused operations (n_fit: bit-exact).  The search rule (O8, round-2 reading) takes no
+decision that rounding noise could flip: a sweep evaluates the six neighbours, takes the first one within
+tol = 1e-12 G of the best and moves only if chi2 drops by more than tol.  So both implementations follow the SAME path
+although they add the points up in different orders: the same number of evaluations, parameters equal to 1e-6,
+chi2 to 1e-9 -- on every fit, noise peaks with flat chi2 included.  The GPU's result is also validated on its own:
+the ORACLE's chi2, depth and level evaluated AT the GPU's parameters are the GPU's."""
 import numpy as np
 import pytest
 
@@ -34,41 +33,39 @@ def run_search(gpu, ctx, b):
 
 
 def compare(orc, star, g, o, p):
-    """g: GPU fit, o: oracle fit, p: the peak.  Returns True if both searches ended at the same point (1e-9)."""
+    """g: GPU fit, o: oracle fit, p: the peak."""
     t, y, dy = star
     D0 = p["m"] / p["nb"] * p["period"]
     assert g["n_fit"] == o["n_fit"] and g["status"] == o["status"]
     if o["status"] != 0:
         assert g["t0"] == o["t0"] and g["q"] == o["q"] and g["q_in"] == o["q_in"]
-        return True
+        return
     floor = 1e-12 * o["chi2_init"]
-    # what is unique: the start value and the minimum reached
     assert abs(g["chi2_init"] - o["chi2_init"]) <= 1e-9 * o["chi2_init"]
-    assert abs(g["chi2"] - o["chi2"]) <= 1e-8 * o["chi2"] + floor
-    # the GPU's parameters are valid: the oracle's chi2, depth and level AT those parameters are the GPU's
+    # the same path: same number of chi2 evaluations, same end point
+    assert int(g["n_eval"]) == int(o["n_eval"]), (int(g["n_eval"]), int(o["n_eval"]))
+    assert abs(g["t0"] - o["t0"]) <= 1e-6 * D0
+    assert abs(g["q"] - o["q"]) <= 1e-6 * o["q"] and abs(g["q_in"] - o["q_in"]) <= 1e-6
+    assert abs(g["chi2"] - o["chi2"]) <= 1e-9 * o["chi2"] + floor
+    scale = max(abs(o["depth"]), 1e-12)
+    assert abs(g["depth"] - o["depth"]) <= 1e-6 * scale and abs(g["z"] - o["z"]) <= 1e-6 * scale + 1e-12 * abs(o["z"])
+    # the GPU's parameters are valid on their own: the oracle's chi2, depth and level AT those parameters
     c2, depth, z = orc.trapezoid_chi2_at(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]),
                                          float(g["t0"] - p["t0"]), float(g["q"]), float(g["q_in"]))
-    scale = max(abs(depth), 1e-12)
     assert abs(g["chi2"] - c2) <= 1e-9 * c2 + floor
-    assert abs(g["depth"] - depth) <= 1e-6 * scale and abs(g["z"] - z) <= 1e-6 * scale + 1e-12 * abs(z)
+    assert abs(g["depth"] - depth) <= 1e-6 * max(abs(depth), 1e-12)
     assert g["chi2"] <= g["chi2_init"] and 0.0 <= g["q"] <= 1.0 and 0.0 <= g["q_in"] <= 0.5
-    assert abs(g["t0"] - p["t0"]) <= D0 and g["n_eval"] <= 605
-    # the parameters themselves: equal when both searches took the same path, else equally good neighbours
-    # (on a noise peak chi2 is flat to ~1e-13 along some directions and the summation order decides a move)
-    assert abs(g["t0"] - o["t0"]) <= 1e-3 * D0
-    assert abs(g["q"] - o["q"]) <= 1e-3 * o["q"] and abs(g["q_in"] - o["q_in"]) <= 2e-3
-    return bool(int(g["n_eval"]) == int(o["n_eval"]) and abs(g["t0"] - o["t0"]) <= 1e-9 * D0 and
-                abs(g["q"] - o["q"]) <= 1e-9 * o["q"] and abs(g["q_in"] - o["q_in"]) <= 1e-9)
+    assert abs(g["t0"] - p["t0"]) <= D0 and g["n_eval"] <= 1205
 
 
-@pytest.mark.parametrize("config,ids", [(1, [0]), (2, list(range(8))), (5, [0, 1, 2, 3, 19, 28])])
+@pytest.mark.parametrize("config,ids", [(1, [0]), (2, list(range(40))), (4, [0, 1]), (5, [0, 1, 2, 3, 19, 28])])
 def test_trapezoid_fit_matches_oracle(gpu, orc, config, ids):
     from paper_2302_01293_b200 import synth
     b = synth.make_batch(config, star_ids=np.array(ids))
     ctx = gpu.QlpBls(top_k=3)
     try:
         pk, fits = run_search(gpu, ctx, b)
-        checked = same_path = 0
+        checked = 0
         for s in range(b.n_stars):
             t, y, dy = b.star(s)
             for r in range(ctx.top_k):
@@ -77,9 +74,9 @@ def test_trapezoid_fit_matches_oracle(gpu, orc, config, ids):
                     assert g["status"] == 1 and g["n_fit"] == 0
                     continue
                 o = orc.trapezoid_fit(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]))
-                same_path += compare(orc, (t, y, dy), g, o, p)
+                compare(orc, (t, y, dy), g, o, p)
                 checked += 1
-        assert checked >= b.n_stars and same_path >= 0.7 * checked
+        assert checked >= b.n_stars
         if config == 1:  # the injected transit of BASELINE.json configs[0]: the fit keeps the BLS depth within 2x
             assert fits[0][0]["status"] == 0 and 0.5 * pk[0][0]["depth"] < fits[0][0]["depth"] < 2.0 * pk[0][0]["depth"]
             assert fits[0][0]["chi2"] < fits[0][0]["chi2_init"]

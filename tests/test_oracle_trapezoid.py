@@ -59,10 +59,12 @@ def test_noise_free_trapezoid_is_recovered(q_in):
     c = make_case(q_in, 0.0, 0)
     r = oracle.trapezoid_fit(c["t"], c["y"], c["dy"], 1.0 / c["P"], c["m"], c["nb"], c["t0_bls"])
     T0, delta, q, qi, z = c["truth"]
-    assert r["status"] == 0 and r["n_eval"] <= 600
+    assert r["status"] == 0 and r["n_eval"] <= 1205
     assert abs(r["t0"] - T0) < 1e-7
     assert abs(r["q"] - q) < 1e-7 and abs(r["q_in"] - qi) < 1e-5
-    assert abs(r["depth"] - delta) < 1e-8 and abs(r["z"] - z) < 1e-9
+    # The search (O8, round-2 reading) stops when no neighbour lowers chi2 by more than 1e-12 G, i.e. at
+    # chi2 ~ 1e-11 G: the linear parameters are then within a few 1e-6 of their scale (depth 0.01, level 1).
+    assert abs(r["depth"] - delta) < 5e-8 and abs(r["z"] - z) < 5e-9
     assert r["chi2"] < 1e-9 * r["chi2_init"]
 
 
@@ -132,3 +134,22 @@ def test_too_few_points_and_flat_data():
     r = oracle.trapezoid_fit(t, y, dy, 1.0 / 2.0, 5, 100, 1.0)      # constant series: nothing to fit
     assert r["status"] == 0 and r["depth"] == 0.0 and r["z"] == pytest.approx(3.0) and r["chi2"] == 0.0
     assert r["q"] == pytest.approx(0.05) and r["q_in"] == 0.25      # no move was accepted
+
+
+@pytest.mark.parametrize("q_in,noise,seed", [(0.2, 0.001, 1), (0.05, 0.001, 2), (0.45, 0.003, 3), (0.3, 0.003, 4),
+                                             (0.25, 0.02, 5), (0.25, 0.05, 6)])
+def test_search_path_is_insensitive_to_rounding_noise(q_in, noise, seed):
+    """The rule of the search (neighbour within tol of the best, move only if chi2 drops by more than tol = 1e-12 G)
+    exists so that rounding noise cannot decide a move.  An affine map of y by numbers that are NOT powers of two
+    changes every rounding error of every sum; the search must take the same path: same number of evaluations, same
+    (T0, q, q_in) to 1e-9 -- also on data that are almost pure noise (the last two cases), where chi2 is flat."""
+    c = make_case(q_in, noise, seed)
+    t, y, dy, P = c["t"], c["y"], c["dy"], c["P"]
+    r0 = oracle.trapezoid_fit(t, y, dy, 1.0 / P, c["m"], c["nb"], c["t0_bls"])
+    for a, b in ((3.0, 0.7), (1.0 / 7.0, -11.3)):
+        r1 = oracle.trapezoid_fit(t, a * y + b, a * dy, 1.0 / P, c["m"], c["nb"], c["t0_bls"])
+        assert r1["n_eval"] == r0["n_eval"]
+        assert abs(r1["t0"] - r0["t0"]) <= 1e-9 * c["m"] / c["nb"] * P
+        assert abs(r1["q"] - r0["q"]) <= 1e-9 * r0["q"] and abs(r1["q_in"] - r0["q_in"]) <= 1e-9
+        assert r1["chi2"] == pytest.approx(r0["chi2"], rel=1e-9)
+        assert r1["depth"] == pytest.approx(a * r0["depth"], rel=1e-6)
