@@ -296,6 +296,13 @@ int qlp_bls_debug_prep(qlp_bls_ctx* ctx, const int64_t* row_ptr, const double* t
                        const double* dy, const qlp_bls_star_grid* grid, int64_t star, double* tau,
                        float* w, float* wy, void* cuda_stream);
 
+/* Bounds-check build only (`python -m paper_2302_01293_b200.build --check` -> libqlp_bls_check.so, compiled with
+ * -DQLP_BOUNDS_CHECK): every guarded shared-memory / workspace access of the fold, scan and fit kernels tests its index
+ * against the extent it must stay in and counts a violation instead of performing the access.  out host uint64[8]:
+ * [0] fold histogram cell, [1] staging chunk, [2] scan bin, [3] fit compaction slot, others reserved; reset != 0
+ * clears the counters.  Synchronises the device.  The normal build returns QLP_BLS_EUNSUPPORTED (and zeros). */
+int qlp_bls_debug_violations(qlp_bls_ctx* ctx, uint64_t* out, int32_t reset);
+
 /* Force the tile class of the fold/scan kernel: 0 = automatic (default); p in 1..9 = no frequency may use a
  * class below p - 1 (class c has 128, 128, 64, 32, 16, 8, 4, 2, 1 columns per CTA for c = 0..8), so that the
  * narrow-column code paths, which real data reach only at very long baselines, are covered on small inputs. */

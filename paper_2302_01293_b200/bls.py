@@ -13,6 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqlp_bls.so")
+LIB_CHECK_PATH = os.path.join(_HERE, "libqlp_bls_check.so")   # bounds-check build (tests only)
 
 
 class QlpBlsError(RuntimeError):
@@ -48,19 +49,20 @@ PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8")
 EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_vet_host", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
            "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_fold_class_counters", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
-           "qlp_bls_debug_set_path"]
+           "qlp_bls_debug_set_path", "qlp_bls_debug_violations"]
 
-_lib = None
+_libs = {}
 
 
-def load_library():
-    """dlopen libqlp_bls.so (built by paper_2302_01293_b200.build); raises if it is missing."""
-    global _lib
-    if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise QlpBlsError(f"{LIB_PATH} not built: run `python -m paper_2302_01293_b200.build` "
-                              "(there is no CPU fallback)")
-        L = C.CDLL(LIB_PATH)
+def load_library(check: bool = False):
+    """dlopen libqlp_bls.so (built by paper_2302_01293_b200.build); raises if it is missing.
+    check=True: the bounds-check build libqlp_bls_check.so (`python -m paper_2302_01293_b200.build --check`)."""
+    path = LIB_CHECK_PATH if check else LIB_PATH
+    if path not in _libs:
+        if not os.path.exists(path):
+            raise QlpBlsError(f"{path} not built: run `python -m paper_2302_01293_b200.build"
+                              f"{' --check' if check else ''}` (there is no CPU fallback)")
+        L = C.CDLL(path)
         vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
         L.qlp_bls_default_config.argtypes = [C.POINTER(Config)]
         L.qlp_bls_default_config.restype = None
@@ -87,8 +89,9 @@ def load_library():
         L.qlp_bls_fold_elapsed_ms.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_double)]
         L.qlp_bls_fold_phase_clocks.argtypes = [vp, vp]
         L.qlp_bls_fold_class_counters.argtypes = [vp, vp]
-        _lib = L
-    return _lib
+        L.qlp_bls_debug_violations.argtypes = [vp, vp, i32]
+        _libs[path] = L
+    return _libs[path]
 
 
 def default_config(**kw) -> Config:
@@ -114,10 +117,10 @@ def _ptr(x):
 class QlpBls:
     """One qlp_bls_ctx.  Methods take/return torch CUDA tensors; nothing is computed in Python."""
 
-    def __init__(self, cfg: Config | None = None, **kw):
+    def __init__(self, cfg: Config | None = None, check: bool = False, **kw):
         import torch
         self.torch = torch
-        self.lib = load_library()
+        self.lib = load_library(check)
         if not torch.cuda.is_available():
             raise QlpBlsError("no CUDA device: the QLP BLS path has no CPU fallback")
         self.cfg = cfg if cfg is not None else default_config(**kw)
@@ -172,6 +175,13 @@ class QlpBls:
         a = np.zeros((9, 5), dtype=np.uint64)
         _check(self.lib.qlp_bls_fold_class_counters(self._h, a.ctypes.data_as(C.c_void_p)),
                "qlp_bls_fold_class_counters")
+        return a
+
+    def debug_violations(self, reset: bool = True) -> np.ndarray:
+        """Bounds-check build only -> uint64[8] violation counters (fold cell, staging, scan bin, fit slot, ...)."""
+        a = np.zeros(8, dtype=np.uint64)
+        _check(self.lib.qlp_bls_debug_violations(self._h, a.ctypes.data_as(C.c_void_p), 1 if reset else 0),
+               "qlp_bls_debug_violations")
         return a
 
     def debug_set_path(self, path: int):

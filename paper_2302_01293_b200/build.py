@@ -13,6 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libqlp_bls.so")
+LIB_CHECK = os.path.join(_HERE, "libqlp_bls_check.so")   # the same sources with -DQLP_BOUNDS_CHECK (tests only)
 UBENCH = os.path.join(_HERE, "qlp_ubench")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
@@ -28,6 +29,16 @@ def needs_build() -> bool:
         return True
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(s) > t for s in sources())
+
+
+def build_check(force: bool = False) -> str:
+    """The bounds-check build (include/qlp_bls.h qlp_bls_debug_violations): same sources, -DQLP_BOUNDS_CHECK."""
+    t = os.path.getmtime(LIB_CHECK) if os.path.exists(LIB_CHECK) else 0.0
+    if force or any(os.path.getmtime(s) > t for s in sources()):
+        nvcc = os.environ.get("NVCC", "nvcc")
+        subprocess.run([nvcc, *NVCC_FLAGS, "-DQLP_BOUNDS_CHECK", "-o", LIB_CHECK, os.path.join(CSRC, "api.cu")],
+                       check=True)
+    return LIB_CHECK
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -46,4 +57,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--check" in sys.argv:
+        print(build_check(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -48,7 +48,7 @@ struct qlp_bls_ctx {
   int32_t force_path = 0;
   int64_t launches = 0;
   // workspace
-  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work, fit_chunk, fit_list, class_ctr;
+  DevBuf pts, prep, kb, cnt, off, counters, star_bins, totals_dev, fit_cnt, fit_off, fit_work, fit_chunk, fit_list, class_ctr, star_order;
   // host-API staging
   DevBuf h_row[2], h_t[2], h_y[2], h_dy[2], h_rho[2], h_grid, h_fptr, h_sr, h_best, h_peaks, h_stats, h_fits, h_pink;
   static const int kSide = 3;           // side streams for the independent tile-class launches
@@ -195,7 +195,7 @@ extern "C" int qlp_bls_destroy(qlp_bls_ctx* ctx) {
   if (!ctx) return QLP_BLS_OK;
   cudaSetDevice(ctx->device);
   DevBuf* bufs[] = {&ctx->pts, &ctx->prep, &ctx->kb, &ctx->cnt, &ctx->off, &ctx->counters, &ctx->star_bins,
-                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->fit_chunk, &ctx->fit_list, &ctx->class_ctr, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
+                    &ctx->totals_dev, &ctx->fit_cnt, &ctx->fit_off, &ctx->fit_work, &ctx->fit_chunk, &ctx->fit_list, &ctx->class_ctr, &ctx->star_order, &ctx->h_row[0], &ctx->h_t[0], &ctx->h_y[0], &ctx->h_dy[0], &ctx->h_rho[0],
                     &ctx->h_row[1], &ctx->h_t[1], &ctx->h_y[1], &ctx->h_dy[1], &ctx->h_rho[1], &ctx->h_grid,
                     &ctx->h_fptr, &ctx->h_sr, &ctx->h_best, &ctx->h_peaks, &ctx->h_stats, &ctx->h_fits, &ctx->h_pink};
   for (DevBuf* b : bufs) b->release();
@@ -463,9 +463,12 @@ extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row
     k.row_ptr = row_ptr; k.t = t; k.y = y; k.dy = dy; k.grid = grid; k.n_stars = n_stars;
     if (!(ctx->prep_valid && ctx->prep_key == k)) QLP_TRY(run_prep(ctx, n_stars, row_ptr, t, y, dy, grid, st));
   }
+  QLP_TRY(ctx->star_order.ensure((size_t)n_stars * sizeof(int32_t)));
+  star_order_kernel<<<1, 1024, 0, st>>>(n_stars, grid, (int32_t*)ctx->star_order.p);
+  QLP_TRY(launch_ok(ctx));
   snr_kernel<<<(unsigned)n_stars, kSnrThreads, kMaxSel * 256 * 4, st>>>(
       ctx->prm, n_stars, row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, grid, freq_ptr, sr, best,
-      snr, peaks);
+      snr, peaks, (const int32_t*)ctx->star_order.p);
   return launch_ok(ctx);
 }
 
@@ -747,6 +750,27 @@ extern "C" int qlp_bls_vet_host(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
                                 void* cuda_stream) {
   return search_host_impl(ctx, n_stars, row_ptr, t, y, dy, rho, rstar, peaks, stats, fits, pink, grid_out, total_freq,
                           cuda_stream);
+}
+
+// ---- check build: violation counters of the guarded accesses (common.cuh QLP_IN_BOUNDS) -------------------------
+extern "C" int qlp_bls_debug_violations(qlp_bls_ctx* ctx, uint64_t* out, int32_t reset) {
+  if (!ctx || !out) return QLP_BLS_EINVAL;
+#ifdef QLP_BOUNDS_CHECK
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  unsigned long long h[kChkSlots];
+  CUDA_TRY(cudaMemcpyFromSymbol(h, g_qlp_violations, sizeof(h)));
+  for (int i = 0; i < kChkSlots; ++i) out[i] = h[i];
+  if (reset) {
+    memset(h, 0, sizeof(h));
+    CUDA_TRY(cudaMemcpyToSymbol(g_qlp_violations, h, sizeof(h)));
+  }
+  return QLP_BLS_OK;
+#else
+  (void)reset;
+  for (int i = 0; i < kChkSlots; ++i) out[i] = 0;
+  return QLP_BLS_EUNSUPPORTED;   // the checks are not compiled into this build
+#endif
 }
 
 // ---- test-only entry points ---------------------------------------------------------------------------

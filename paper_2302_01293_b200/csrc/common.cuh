@@ -54,6 +54,19 @@ struct Params {
 };
 
 
+// ---- optional bounds checks (the `check` build: -DQLP_BOUNDS_CHECK -> libqlp_bls_check.so) --------------------
+// compute-sanitizer is closed on the GPU pool this library is developed on, so the shared-memory and workspace
+// indices of the kernels can be checked by a build of their own: every guarded access tests its index against the
+// extent it must stay in, counts a violation (per site class) instead of performing the access, and
+// qlp_bls_debug_violations() reads the counters back.  In the normal build the macros cost nothing.
+enum { kChkFoldCell = 0, kChkStage = 1, kChkScanBin = 2, kChkFitSlot = 3, kChkSnr = 4, kChkSlots = 8 };
+#ifdef QLP_BOUNDS_CHECK
+__device__ unsigned long long g_qlp_violations[kChkSlots];
+#define QLP_IN_BOUNDS(slot, cond) ((cond) ? true : (atomicAdd(&g_qlp_violations[slot], 1ull), false))
+#else
+#define QLP_IN_BOUNDS(slot, cond) (true)
+#endif
+
 // ---- exact FP64 helpers: never contracted into FMAs (O1/O3: "no fused multiply-add") ---
 __device__ __forceinline__ double dmul(double a, double b) { return __dmul_rn(a, b); }
 __device__ __forceinline__ double dadd(double a, double b) { return __dadd_rn(a, b); }

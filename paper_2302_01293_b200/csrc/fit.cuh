@@ -325,8 +325,11 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
       const int p = pos + before + __popc(bal & ((1u << lane) - 1u));
       const double d = dy[a + i];
       const double wi = 1.0 / (d * d);
-      if (p < kFitCap) { sdt[p] = dt; sy[p] = y[a + i]; sw[p] = wi; }
-      else { dtv[p] = dt; yv[p] = y[a + i]; wv[p] = wi; }
+      // check build: the slot lies inside this CTA's share of the window (the counts of fit_count_kernel)
+      if (QLP_IN_BOUNDS(kChkFitSlot, p >= 0 && p < cnt && base + p < nf)) {
+        if (p < kFitCap) { sdt[p] = dt; sy[p] = y[a + i]; sw[p] = wi; }
+        else { dtv[p] = dt; yv[p] = y[a + i]; wv[p] = wi; }
+      }
     }
     pos += total;
     cb ^= 1;

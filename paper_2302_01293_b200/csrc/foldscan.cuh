@@ -277,6 +277,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         mbar_wait(&mbar[b], (b ? use1 : use0) & 1u);
         if (b) ++use1; else ++use0;
         const int64_t left = n - c * kChunk;
+        (void)QLP_IN_BOUNDS(kChkStage, left > 0 && b >= 0 && b < 2);
         if (left < kChunk) {  // pad the tail with weightless points so that every chunk is full
           for (int i = (int)left + tid; i < kChunk; i += kThreads) {
             Point z; z.tau = 0.0; z.W = 0u; z.S = 0;
@@ -300,6 +301,10 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
               bin_parts(f[r], tau, dnb[r], I, g);
               const uint32_t off = g * neg_nb_row[r] + (I * (uint32_t)(STRIDE * 4) + lane_off);
               uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + 32 * r;
+              // check build: the row of the cell lies inside this tile's histogram (bin < nb of the column <= nb_tile)
+              if (!QLP_IN_BOUNDS(kChkFoldCell, off / (uint32_t)(STRIDE * 4) < (uint32_t)nb_tile &&
+                                                   (off % (uint32_t)(STRIDE * 4)) / 4u + 32u * r < (uint32_t)CTOT))
+                continue;
               if (HPW == 1) {
                 atomicAdd(cell, (uint32_t)v[u].z);
                 atomicAdd(cell + CTOT, (uint32_t)v[u].w);
@@ -365,6 +370,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
             if (j < jb) {
               int e = j + MW - 1;
               if (e >= nbk) e -= nbk;
+              if (!QLP_IN_BOUNDS(kChkScanBin, e >= 0 && e < nbk && nbk <= nb_tile)) e = 0;
               ww[(jj + MW - 1) % MW] = (float)hc[e * STRIDE] * inv_w;
               ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * STRIDE + CTOT];
               float r = 0.f, sm = 0.f, vj = 0.f;

@@ -4,15 +4,39 @@
 
 namespace qlp {
 
+// Stars in order of decreasing grid size (by power-of-two bucket of n_freq): snr_kernel is one CTA per star and the
+// hardware hands out CTAs in index order, so with the longest grids first a 5e5-frequency star does not end up as a
+// lone tail while the other SMs idle.  One CTA: count per bucket, scan, scatter (the order inside a bucket is
+// whatever the atomics give -- it only decides which CTA runs when, never a result).
+__global__ void __launch_bounds__(1024) star_order_kernel(int64_t n_stars, const qlp_bls_star_grid* __restrict__ grid,
+                                                          int32_t* __restrict__ order) {
+  __shared__ unsigned int cnt[64], base[64];
+  if (threadIdx.x < 64) cnt[threadIdx.x] = 0u;
+  __syncthreads();
+  auto bucket = [&](int64_t s) {
+    const qlp_bls_star_grid g = grid[s];
+    const long long n = g.status == 0 ? (long long)g.n_freq : 0;
+    return n > 0 ? 63 - __clzll(n) + 1 : 0;               // 0: nothing to do; larger = longer grid
+  };
+  for (int64_t s = threadIdx.x; s < n_stars; s += blockDim.x) atomicAdd(&cnt[bucket(s)], 1u);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned int acc = 0;
+    for (int b = 63; b >= 0; --b) { base[b] = acc; acc += cnt[b]; }
+  }
+  __syncthreads();
+  for (int64_t s = threadIdx.x; s < n_stars; s += blockDim.x) order[atomicAdd(&base[bucket(s)], 1u)] = (int32_t)s;
+}
+
 __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
     Params prm, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const float* __restrict__ sr, const uint32_t* __restrict__ best,
-    float* __restrict__ snr_out, qlp_bls_peak* __restrict__ peaks) {
+    float* __restrict__ snr_out, qlp_bls_peak* __restrict__ peaks, const int32_t* __restrict__ order) {
   extern __shared__ __align__(16) uint32_t sel_hist[];  // kMaxSel * 256 counters
   __shared__ SnrShared sh;
-  const int64_t s = blockIdx.x;
-  if (s >= n_stars) return;
+  if ((int64_t)blockIdx.x >= n_stars) return;
+  const int64_t s = order[blockIdx.x];                   // longest grids first (star_order_kernel)
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int K = prm.top_k;
   const qlp_bls_star_grid g = grid[s];
