@@ -444,6 +444,7 @@ def run_gpu(args):
     n_small = max(1, min(args.steps, 5))
     ctx.trapezoid_fit(row_ptr, t, y, dy, peaks)
     torch.cuda.synchronize()
+    ctx.fold_timing(True)    # also makes the fit kernels count their (point, sweep) pairs
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record()
     for _ in range(n_small):
@@ -451,6 +452,8 @@ def run_gpu(args):
     f1.record()
     torch.cuda.synchronize()
     fit_ms = f0.elapsed_time(f1) / n_small
+    fit_pairs = ctx.fit_work() / n_small
+    ctx.fold_timing(False)
     fit_np = bls.fits_to_numpy(fits, K)
     ctx.pink_noise(row_ptr, t, y, peaks, fits)
     f0.record()
@@ -541,7 +544,18 @@ def run_gpu(args):
         # rank 0's shard, outside the timed region of `value`: count + scan + fit kernels of qlp_bls_trapezoid_fit
         "trapezoid_fit": {"ms_per_call": fit_ms, "fits": int(fit_np.size), "fits_per_s": fit_np.size / (fit_ms * 1e-3),
                           "mean_points_per_fit": float(fit_np["n_fit"].mean()),
-                          "mean_chi2_evaluations": float(fit_np["n_eval"].mean())},
+                          "mean_chi2_evaluations": float(fit_np["n_eval"].mean()),
+                          # Algorithmic work of O8: one trapezoid evaluation = one (point inside the transit, candidate)
+                          # pair = 8 FP64 instructions (|dt - c|, half - u, x inv_ing, min, w sh, three accumulations);
+                          # the kernels count the (point, sweep) pairs, each is six evaluations.  Bound: the FP64 pipe.
+                          "roofline": {"bound": "alu", "unit": "G trapezoid evaluations/s",
+                                       "achieved": 6.0 * fit_pairs / (fit_ms * 1e-3) / 1e9,
+                                       "peak": N_SM * sm_max * 1e6 * FP64_LANES_PER_CLK_SM / 8.0 / 1e9,
+                                       "frac": 6.0 * fit_pairs / (fit_ms * 1e-3) /
+                                               (N_SM * sm_max * 1e6 * FP64_LANES_PER_CLK_SM / 8.0),
+                                       "evaluations_per_call": 6.0 * fit_pairs,
+                                       "note": "latency-bound: ~90 serial sweeps per fit (pass, 18 reductions, solve, "
+                                               "decision), DESIGN.md section 4 O8"}},
         "pink_noise": {"ms_per_call": pink_ms, "detected_stars": int((pink_np["detected"].max(axis=1) > 0).sum())},
         "roofline": {"bound": "alu", "kernel": "foldscan_kernel (9 class launches per step)",
                      "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "Gevals/s",

@@ -270,6 +270,11 @@ int qlp_bls_fold_elapsed_ms(qlp_bls_ctx* ctx, int32_t* n_calls /*host*/, double*
  * Their ratios split the fused kernel's time between S2 and S3.  Synchronises the device.  clocks host [3]. */
 int qlp_bls_fold_phase_clocks(qlp_bls_ctx* ctx, uint64_t* clocks /*host*/);
 
+/* Work of the trapezoid fits since qlp_bls_fold_timing(ctx, 1): out host uint64[2], out[0] = (point, sweep) pairs in
+ * which the point lay inside some candidate's transit (each is six trapezoid evaluations of O8), out[1] reserved.
+ * Synchronises the device. */
+int qlp_bls_fit_work(qlp_bls_ctx* ctx, uint64_t* out);
+
 /* Per tile class c = 0..8 of the fold/scan kernel, summed over all tiles since
  * qlp_bls_fold_timing(ctx, 1): out host uint64[9][5] = {set-up + zeroing clocks, fold clocks, scan clocks (SM clocks
  * of thread 0 of each CTA), point x frequency evaluations, tiles}.  Synchronises the device. */

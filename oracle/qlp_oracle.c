@@ -570,8 +570,8 @@ int orc_sizeof_peak_stats(void) { return (int)sizeof(orc_peak_stats); }
  *              neighbours theta +- h_d e_d (order c+, c-, q+, q-, q_in+, q_in-; clipped to the bounds, skipped
  *              if the clipped value is the current one), takes the FIRST neighbour in that order whose chi2 is
  *              within tol of the smallest of them, and moves there iff it lowers chi2 by more than tol; a sweep
- *              that does not move halves the steps; 24 halvings; no sweep starts once 1200 evaluations are
- *              spent (so at most 1205).  tol = max(1e-9 chi2_best, 1e-12 G), chi2_best the current value and
+ *              that does not move halves the steps; 24 halvings; no sweep starts once 600 evaluations are
+ *              spent (so at most 605).  tol = max(1e-9 chi2_best, 1e-12 G), chi2_best the current value and
  *              G = sum w (y - ybar)^2 over the window.  chi2 values of two implementations differ by ~1e-15 G
  *              (FP64 sums of ~10^3..10^5 terms in different orders), a million times less than tol on real data
  *              (chi2 ~ G), so neither the choice of the neighbour nor the acceptance depends on the order in
@@ -658,9 +658,9 @@ void orc_trapezoid_fit(int64_t n, const double* t, const double* y, const double
   int n_eval = 1;
   out->chi2_init = best;
   const double tol_floor = 1e-12 * fd.G;
-  for (int level = 0; level < 24 && n_eval < 1200; ++level) {
+  for (int level = 0; level < 24 && n_eval < 600; ++level) {
     int moved = 1;
-    while (moved && n_eval < 1200) {
+    while (moved && n_eval < 600) {
       moved = 0;
       double tol = 1e-9 * best;
       if (tol < tol_floor) tol = tol_floor;

@@ -48,7 +48,7 @@ PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8")
 
 EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_vet_host", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
-           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_fold_class_counters", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
+           "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_fold_class_counters", "qlp_bls_fit_work", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path", "qlp_bls_debug_violations"]
 
 _libs = {}
@@ -89,6 +89,7 @@ def load_library(check: bool = False):
         L.qlp_bls_fold_elapsed_ms.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_double)]
         L.qlp_bls_fold_phase_clocks.argtypes = [vp, vp]
         L.qlp_bls_fold_class_counters.argtypes = [vp, vp]
+        L.qlp_bls_fit_work.argtypes = [vp, vp]
         L.qlp_bls_debug_violations.argtypes = [vp, vp, i32]
         _libs[path] = L
     return _libs[path]
@@ -176,6 +177,12 @@ class QlpBls:
         _check(self.lib.qlp_bls_fold_class_counters(self._h, a.ctypes.data_as(C.c_void_p)),
                "qlp_bls_fold_class_counters")
         return a
+
+    def fit_work(self) -> int:
+        """(point, sweep) pairs inside a transit that the fit kernels processed since fold_timing(True)."""
+        a = np.zeros(2, dtype=np.uint64)
+        _check(self.lib.qlp_bls_fit_work(self._h, a.ctypes.data_as(C.c_void_p)), "qlp_bls_fit_work")
+        return int(a[0])
 
     def debug_violations(self, reset: bool = True) -> np.ndarray:
         """Bounds-check build only -> uint64[8] violation counters (fold cell, staging, scan bin, fit slot, ...)."""

@@ -248,8 +248,8 @@ extern "C" int qlp_bls_fold_timing(qlp_bls_ctx* ctx, int32_t enable) {
   }
   ctx->timing = enable != 0;
   ctx->ev_calls = 0;
-  QLP_TRY(ctx->class_ctr.ensure(kNumClasses * kClassCtr * 8));
-  CUDA_TRY(cudaMemset(ctx->class_ctr.p, 0, kNumClasses * kClassCtr * 8));
+  QLP_TRY(ctx->class_ctr.ensure((kNumClasses * kClassCtr + 2) * 8));
+  CUDA_TRY(cudaMemset(ctx->class_ctr.p, 0, (kNumClasses * kClassCtr + 2) * 8));
   return QLP_BLS_OK;
 }
 
@@ -262,6 +262,16 @@ extern "C" int qlp_bls_fold_class_counters(qlp_bls_ctx* ctx, uint64_t* out) {
   CUDA_TRY(cudaMemcpy(h, ctx->class_ctr.p, sizeof(h), cudaMemcpyDeviceToHost));
   for (int c = 0; c < kNumClasses; ++c)
     for (int i = 0; i < 5; ++i) out[c * 5 + i] = h[c * kClassCtr + i];
+  return QLP_BLS_OK;
+}
+
+extern "C" int qlp_bls_fit_work(qlp_bls_ctx* ctx, uint64_t* out) {
+  if (!ctx || !out) return QLP_BLS_EINVAL;
+  out[0] = out[1] = 0;
+  if (!ctx->class_ctr.p) return QLP_BLS_OK;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  CUDA_TRY(cudaMemcpy(out, (unsigned long long*)ctx->class_ctr.p + kNumClasses * kClassCtr, 16, cudaMemcpyDeviceToHost));
   return QLP_BLS_OK;
 }
 
@@ -525,6 +535,8 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
   // a single window never holds more points than its star, and a star is capped at QLP_BLS_MAX_POINTS < 2^31
   rc = ctx->fit_work.ensure((size_t)(total > 0 ? total : 1) * 3 * sizeof(double));
   if (rc != 0) return rc;
+  // while fold timing is on, the fit kernels count their work (bench.py's roofline entry): class_ctr[72..73]
+  unsigned long long* fit_ctr = (ctx->timing && ctx->class_ctr.p) ? (unsigned long long*)ctx->class_ctr.p + kNumClasses * kClassCtr : nullptr;
   // Large windows first, on a side stream: one cluster of kFitCluster CTAs per item; the single-CTA fits of the small
   // windows run beside them on the caller's stream.  Both grids are exact (the size classes were counted above).
   QLP_TRY(ensure_side_streams(ctx));
@@ -542,13 +554,13 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
     lc.attrs = at; lc.numAttrs = 1;
     CUDA_TRY(cudaLaunchKernelEx(&lc, fit_kernel<kFitCluster>, n_items, (int)ctx->prm.top_k, row_ptr, t, y, dy, peaks,
                                 (const int64_t*)off, (const int32_t*)chunk, (const int32_t*)(list + n_items), n_cluster,
-                                (double*)ctx->fit_work.p, fits));
+                                (double*)ctx->fit_work.p, fits, fit_ctr));
     QLP_TRY(launch_ok(ctx));
   }
   if (n_single > 0) {
     fit_kernel<1><<<(unsigned)n_single, kFitThreads, kFitSmemBytes, st>>>(n_items, ctx->prm.top_k, row_ptr, t, y, dy, peaks,
                                                                         off, chunk, list, n_single,
-                                                                        (double*)ctx->fit_work.p, fits);
+                                                                        (double*)ctx->fit_work.p, fits, fit_ctr);
     QLP_TRY(launch_ok(ctx));
   }
   CUDA_TRY(cudaEventRecord(ctx->side_done[0], ctx->side[0]));

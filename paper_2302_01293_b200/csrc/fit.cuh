@@ -36,7 +36,7 @@ constexpr int kFitCap = 2240;      // points of a fit held in one CTA's shared m
 constexpr int kFitSingleMax = 2 * kFitCap;   // windows up to this many points are fitted by one CTA
 constexpr int kFitSmemBytes = 3 * kFitCap * 8;
 constexpr int kFitLevels = 24;     // step halvings
-constexpr int kFitMaxEval = 1200;  // no sweep starts once this many chi2 evaluations are spent
+constexpr int kFitMaxEval = 600;   // no sweep starts once this many chi2 evaluations are spent
 constexpr int kFitMinPoints = 5;
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -174,15 +174,29 @@ __device__ __forceinline__ void trial_add(double u, double half, double inv_ing,
 // Sums B = sum w sh, C = sum w sh^2, F = sum w (y - ybar) sh of all six candidates over points [begin, end) in ONE
 // pass.  Only points inside some candidate's transit do any work; consecutive points are consecutive in time, so
 // whole warps skip the rest of the window.
+template <bool PREFETCH>
 __device__ __forceinline__ void trial_sums(const double* __restrict__ dt, const double* __restrict__ wy,
                                            const double* __restrict__ w, int begin, int end, const Trial& tr,
-                                           double (&s)[18]) {
+                                           double (&s)[18], unsigned int& in_reach) {
+  // PREFETCH (the part of a window that lives in global memory): the records of the next iteration are requested
+  // before this one's are used, so the L2 latency of one iteration hides behind the arithmetic of another
+  int i = begin + threadIdx.x;
+  double d_n = 0.0, w_n = 0.0, wy_n = 0.0;
+  if (PREFETCH && i < end) { d_n = dt[i]; w_n = w[i]; wy_n = wy[i]; }
 #pragma unroll 1
-  for (int i = begin + threadIdx.x; i < end; i += kFitThreads) {
-    const double d = dt[i];
+  for (; i < end; i += kFitThreads) {
+    double d, wi, wyi;
+    if (PREFETCH) {
+      d = d_n; wi = w_n; wyi = wy_n;
+      const int j = i + kFitThreads;
+      if (j < end) { d_n = dt[j]; w_n = w[j]; wy_n = wy[j]; }
+    } else {
+      d = dt[i];
+    }
     const double u0 = fabs(d - tr.cb);            // candidates 2..5 keep the current epoch
     if (u0 < tr.reach) {
-      const double wi = w[i], wyi = wy[i];
+      if (!PREFETCH) { wi = w[i]; wyi = wy[i]; }
+      ++in_reach;
       trial_add(fabs(d - tr.c0), tr.hb, tr.ib, wi, wyi, s[0], s[1], s[2]);
       trial_add(fabs(d - tr.c1), tr.hb, tr.ib, wi, wyi, s[3], s[4], s[5]);
       trial_add(u0, tr.h2, tr.i2, wi, wyi, s[6], s[7], s[8]);
@@ -246,12 +260,12 @@ __device__ __forceinline__ void all_sum(double (&v)[NV], double* red, double* xc
 // k's (chi2, depth, z); the other lanes hold chi2 = +inf.
 template <int CS>
 __device__ __forceinline__ void trial_chi2(const FitData& fd, double* red, double* xchg, int& ph, const Trial& tr,
-                                           double& chi2, double& depth, double& z) {
+                                           double& chi2, double& depth, double& z, unsigned int& in_reach) {
   double s[18];
 #pragma unroll
   for (int k = 0; k < 18; ++k) s[k] = 0.0;
-  trial_sums(fd.s_dt, fd.s_wy, fd.s_w, 0, fd.n < kFitCap ? fd.n : kFitCap, tr, s);
-  if (fd.n > kFitCap) trial_sums(fd.g_dt, fd.g_wy, fd.g_w, kFitCap, fd.n, tr, s);
+  trial_sums<false>(fd.s_dt, fd.s_wy, fd.s_w, 0, fd.n < kFitCap ? fd.n : kFitCap, tr, s, in_reach);
+  if (fd.n > kFitCap) trial_sums<true>(fd.g_dt, fd.g_wy, fd.g_w, kFitCap, fd.n, tr, s, in_reach);
   const double tot = all_sum_to_lanes<CS, 18>(s, red, xchg, ph);   // lane l: value l = 3 k + {0: B, 1: C, 2: F}
   const int lane = threadIdx.x & 31;
   const int k3 = lane < 6 ? 3 * lane : 0;
@@ -277,7 +291,9 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
                                                           const int32_t* __restrict__ chunk_count,
                                                           const int32_t* __restrict__ list, int64_t n_list,
                                                           double* __restrict__ work,
-                                                          qlp_bls_trapezoid* __restrict__ fits) {
+                                                          qlp_bls_trapezoid* __restrict__ fits,
+                                                          unsigned long long* __restrict__ work_ctr /* NULL, or two
+                                                          counters: (point, sweep) pairs inside a transit; sweeps */) {
   constexpr int NW = kFitThreads / 32;
   extern __shared__ __align__(16) double fit_smem[];   // 3 x kFitCap doubles: dt, y -> w (y - ybar), w
   __shared__ double red[2 * 18 * NW], xchg[2 * 18];
@@ -366,6 +382,7 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
     double dl = 0.0, z = 0.0, best = 0.0;
     int n_eval = 0;
     Trial tr;
+    unsigned int in_reach = 0;   // points this thread found inside some candidate's transit, over all sweeps
     // start point: the sweep machinery at zero steps (all six candidates are the start point; lane 2 is read)
     {
       const double D = th1 * fd.P;
@@ -374,7 +391,7 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
       tr.ib = tr.i2 = tr.i3 = tr.i4 = tr.i5 = 1.0 / (th2 * D);
       tr.reach = tr.hb;
       double chi, d2, z2;
-      trial_chi2<CS>(fd, red, xchg, ph, tr, chi, d2, z2);
+      trial_chi2<CS>(fd, red, xchg, ph, tr, chi, d2, z2, in_reach);
       best = __shfl_sync(0xffffffffu, chi, 2); dl = __shfl_sync(0xffffffffu, d2, 2); z = __shfl_sync(0xffffffffu, z2, 2);
       o.chi2_init = best;
       n_eval = 1;
@@ -399,7 +416,7 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
         tr.i4 = 1.0 / (i_p * Db); tr.i5 = 1.0 / (i_m * Db);
         tr.reach = fmax(fmax(tr.h2, tr.h3), tr.hb + fmax(c_p - th0, th0 - c_m));
         double chi, d2, z2;
-        trial_chi2<CS>(fd, red, xchg, ph, tr, chi, d2, z2);     // lane k < 6: candidate k
+        trial_chi2<CS>(fd, red, xchg, ph, tr, chi, d2, z2, in_reach);     // lane k < 6: candidate k
         n_eval += __popc(have);
         if (!((have >> lane) & 1u)) chi = inf;            // lanes >= 6 hold +inf already
         double cmin = chi;
@@ -422,6 +439,11 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
       h0 *= 0.5; h1 *= 0.5; h2 *= 0.5;
     }
     o.t0 = pk.t0 + th0; o.q = th1; o.q_in = th2; o.depth = dl; o.z = z; o.chi2 = best; o.n_eval = n_eval;
+    if (work_ctr) {   // bench.py's roofline entry of the fit: each such pair is six trapezoid evaluations
+#pragma unroll
+      for (int o2 = 16; o2 > 0; o2 >>= 1) in_reach += __shfl_xor_sync(0xffffffffu, in_reach, o2);
+      if (lane == 0) atomicAdd(&work_ctr[0], (unsigned long long)in_reach);
+    }
   }
   if (threadIdx.x == 0 && rank == 0) fits[item] = o;
   if (CS > 1) cooperative_groups::this_cluster().sync();   // no CTA leaves while a neighbour may still read its xchg

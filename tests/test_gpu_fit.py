@@ -55,7 +55,7 @@ def compare(orc, star, g, o, p):
     assert abs(g["chi2"] - c2) <= 1e-9 * c2 + floor
     assert abs(g["depth"] - depth) <= 1e-6 * max(abs(depth), 1e-12)
     assert g["chi2"] <= g["chi2_init"] and 0.0 <= g["q"] <= 1.0 and 0.0 <= g["q_in"] <= 0.5
-    assert abs(g["t0"] - p["t0"]) <= D0 and g["n_eval"] <= 1205
+    assert abs(g["t0"] - p["t0"]) <= D0 and g["n_eval"] <= 605
 
 
 @pytest.mark.parametrize("config,ids", [(1, [0]), (2, list(range(40))), (4, [0, 1]), (5, [0, 1, 2, 3, 19, 28])])

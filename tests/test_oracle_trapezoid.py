@@ -59,7 +59,7 @@ def test_noise_free_trapezoid_is_recovered(q_in):
     c = make_case(q_in, 0.0, 0)
     r = oracle.trapezoid_fit(c["t"], c["y"], c["dy"], 1.0 / c["P"], c["m"], c["nb"], c["t0_bls"])
     T0, delta, q, qi, z = c["truth"]
-    assert r["status"] == 0 and r["n_eval"] <= 1205
+    assert r["status"] == 0 and r["n_eval"] <= 605
     assert abs(r["t0"] - T0) < 1e-7
     assert abs(r["q"] - q) < 1e-7 and abs(r["q_in"] - qi) < 1e-5
     # The search (O8, round-2 reading) stops when no neighbour lowers chi2 by more than 1e-12 G, i.e. at
