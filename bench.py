@@ -369,6 +369,9 @@ def run_gpu(args):
     use_dist = world > 1 or os.environ.get("QLP_BENCH_FORCE_DIST") == "1"  # the latter: exercise NCCL at world 1
     device = f"cuda:{local}"
     if use_dist:
+        if "RANK" not in os.environ:   # QLP_BENCH_FORCE_DIST outside torchrun: a one-rank group on this host
+            os.environ.update(RANK="0", WORLD_SIZE="1", LOCAL_RANK="0", MASTER_ADDR="127.0.0.1",
+                              MASTER_PORT=os.environ.get("MASTER_PORT", "29533"))
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
         build.build()
@@ -545,6 +548,12 @@ def run_gpu(args):
         "trapezoid_fit": {"ms_per_call": fit_ms, "fits": int(fit_np.size), "fits_per_s": fit_np.size / (fit_ms * 1e-3),
                           "mean_points_per_fit": float(fit_np["n_fit"].mean()),
                           "mean_chi2_evaluations": float(fit_np["n_eval"].mean()),
+                          "chi2_evaluations_p50_p90_max": [float(np.percentile(fit_np["n_eval"], 50)),
+                                                           float(np.percentile(fit_np["n_eval"], 90)),
+                                                           float(fit_np["n_eval"].max())],
+                          "points_per_fit_p50_p90_max": [float(np.percentile(fit_np["n_fit"], 50)),
+                                                         float(np.percentile(fit_np["n_fit"], 90)),
+                                                         float(fit_np["n_fit"].max())],
                           # Algorithmic work of O8: one trapezoid evaluation = one (point inside the transit, candidate)
                           # pair = 8 FP64 instructions (|dt - c|, half - u, x inv_ing, min, w sh, three accumulations);
                           # the kernels count the (point, sweep) pairs, each is six evaluations.  Bound: the FP64 pipe.

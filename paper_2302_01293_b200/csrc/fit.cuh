@@ -33,7 +33,7 @@ constexpr int kFitWarps = 4;       // (star, peak) items per CTA of the counting
 constexpr int kFitThreads = 128;   // threads of one CTA of the fit kernel (128 registers each: four CTAs per SM)
 constexpr int kFitCluster = 8;     // CTAs per cluster for large windows (portable cluster size)
 constexpr int kFitCap = 2240;      // points of a fit held in one CTA's shared memory (52.5 KB: four CTAs per SM)
-constexpr int kFitSingleMax = 2 * kFitCap;   // windows up to this many points are fitted by one CTA
+constexpr int kFitSingleMax = 4 * kFitCap;   // windows up to this many points are fitted by one CTA (measured best)
 constexpr int kFitSmemBytes = 3 * kFitCap * 8;
 constexpr int kFitLevels = 24;     // step halvings
 constexpr int kFitMaxEval = 600;   // no sweep starts once this many chi2 evaluations are spent
@@ -412,8 +412,14 @@ __global__ void __launch_bounds__(kFitThreads, 4) fit_kernel(int64_t n_items, in
         const double Db = th1 * fd.P, D2 = q_p * fd.P, D3 = q_m * fd.P;
         tr.c0 = c_p; tr.c1 = c_m; tr.cb = th0;
         tr.hb = 0.5 * Db; tr.h2 = 0.5 * D2; tr.h3 = 0.5 * D3;
-        tr.ib = 1.0 / (th2 * Db); tr.i2 = 1.0 / (th2 * D2); tr.i3 = 1.0 / (th2 * D3);
-        tr.i4 = 1.0 / (i_p * Db); tr.i5 = 1.0 / (i_m * Db);
+        {  // the five reciprocals 1 / ingress, one FP64 division per lane instead of five in every lane
+          const double den = lane == 0 ? th2 * Db : lane == 1 ? th2 * D2 : lane == 2 ? th2 * D3
+                           : lane == 3 ? i_p * Db : i_m * Db;
+          const double inv = 1.0 / den;
+          tr.ib = __shfl_sync(0xffffffffu, inv, 0); tr.i2 = __shfl_sync(0xffffffffu, inv, 1);
+          tr.i3 = __shfl_sync(0xffffffffu, inv, 2); tr.i4 = __shfl_sync(0xffffffffu, inv, 3);
+          tr.i5 = __shfl_sync(0xffffffffu, inv, 4);
+        }
         tr.reach = fmax(fmax(tr.h2, tr.h3), tr.hb + fmax(c_p - th0, th0 - c_m));
         double chi, d2, z2;
         trial_chi2<CS>(fd, red, xchg, ph, tr, chi, d2, z2, in_reach);     // lane k < 6: candidate k
