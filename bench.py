@@ -206,7 +206,10 @@ def make_times_ids(config: int, ids, pool, block: int = 500):
 # ---------------------------------------------------------------------------------------------- the oracle, timed
 GRID_NOTE = "comparison grid O1.10 (PAPER.md:13): P <= 56 d, <= 80,000 frequencies per star"
 GRID_KW = {}   # --comparison-grid: the O1.10 caps, given to both the CUDA context and the oracle config
-ORACLE_KIND = "oracle (the unoptimised FP64 checker of oracle/: triple-loop box scan, 128-bit bin index; not a tuned CPU BLS)"
+ORACLE_KIND = "oracle"
+ORACLE_NOTE = ("the unoptimised FP64 checker of oracle/ as it stands (triple-loop box scan, 128-bit bin index, malloc per "
+               "star): a reported baseline, not a tuned CPU BLS; a GPU/CPU ratio formed from it says nothing about "
+               "kernel quality")
 
 
 class OracleSample:
@@ -276,7 +279,7 @@ def cpu_baseline(batch, budget_s: float = 15.0):
     cores = os.cpu_count() or 1
     smp = OracleSample(batch, budget_s, cores)
     dt, ev = smp.run()
-    return {"value": ev / dt, "unit": UNIT, "cores": cores, "kind": ORACLE_KIND,
+    return {"value": ev / dt, "unit": UNIT, "cores": cores, "kind": ORACLE_KIND, "note": ORACLE_NOTE,
             "sample": f"{smp.desc}, {dt:.1f} s", "seconds": dt}
 
 
@@ -308,7 +311,8 @@ def run_reference(args):
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
            "config": {"workload": f"config{args.config}: bounded sample of BASELINE.json configs[{args.config - 1}] "
                                   f"({sample})", **({"grid": GRID_NOTE} if GRID_KW else {})},
-           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": ORACLE_KIND, "sample": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": ORACLE_KIND, "note": ORACLE_NOTE,
+                            "sample": sample},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     emit(json.dumps(out))
@@ -472,8 +476,7 @@ def run_gpu(args):
     torch.cuda.empty_cache()
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
     h = [pin(batch.row_ptr), pin(batch.t), pin(batch.y), pin(batch.dy), pin(batch.rho)]
-    n_warm = min(S, 200)   # staging buffers, streams
-    ctx.search_host(h[0][:n_warm + 1], h[1], h[2], h[3], h[4][:n_warm], want_stats=True)
+    ctx.search_host(*h, want_stats=True)   # untimed: staging buffers of the full size, streams
     barrier()
     t0 = time.perf_counter()
     for _ in range(n_small):
@@ -485,7 +488,7 @@ def run_gpu(args):
     e2e_s = (time.perf_counter() - t0) / n_small
     h2d = int(sum(a.nbytes for a in h))
     d2h = int(pk_host.nbytes + st_host.nbytes)
-    ctx.vet_host(h[0][:n_warm + 1], h[1], h[2], h[3], h[4][:n_warm])
+    ctx.vet_host(*h)                       # untimed: the fit workspace of the full size
     barrier()
     t0 = time.perf_counter()
     for _ in range(n_small):

@@ -519,8 +519,7 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
   // two counters (items per size class) behind the lists, 8-byte aligned
   unsigned long long* list_n = (unsigned long long*)((char*)ctx->fit_list.p + (((size_t)n_items * 2 * sizeof(int32_t) + 7) & ~(size_t)7));
   CUDA_TRY(cudaMemsetAsync(list_n, 0, 16, st));
-  const unsigned n_cta = (unsigned)((n_items + kFitWarps - 1) / kFitWarps);
-  fit_count_kernel<<<n_cta, kFitWarps * 32, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, peaks, cnt, chunk, list, list_n);
+  fit_count_kernel<<<(unsigned)n_items, kFitCountThreads, 0, st>>>(n_items, ctx->prm.top_k, row_ptr, t, peaks, cnt, chunk, list, list_n);
   rc = launch_ok(ctx);
   if (rc != 0) return rc;
   fit_scan_kernel<<<1, 1024, 0, st>>>(n_items, cnt, off, off + n_items + 1);

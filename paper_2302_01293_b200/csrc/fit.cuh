@@ -29,7 +29,7 @@
 
 namespace qlp {
 
-constexpr int kFitWarps = 4;       // (star, peak) items per CTA of the counting kernel
+constexpr int kFitCountThreads = 256;   // threads of the CTA that counts the window points of one (star, peak)
 constexpr int kFitThreads = 128;   // threads of one CTA of the fit kernel (128 registers each: four CTAs per SM)
 constexpr int kFitCluster = 8;     // CTAs per cluster for large windows (portable cluster size)
 constexpr int kFitCap = 2240;      // points of a fit held in one CTA's shared memory (52.5 KB: four CTAs per SM)
@@ -68,33 +68,38 @@ __device__ __forceinline__ double fit_dt(double t, const FitWindow& w) {
 // chunk r of a star of n points: [n r / kFitCluster, n (r + 1) / kFitCluster)
 __device__ __forceinline__ int64_t fit_chunk_begin(int64_t n, int r) { return (n * r) / kFitCluster; }
 
-__global__ void __launch_bounds__(kFitWarps * 32) fit_count_kernel(int64_t n_items, int top_k,
-                                                                   const int64_t* __restrict__ row_ptr,
-                                                                   const double* __restrict__ t,
-                                                                   const qlp_bls_peak* __restrict__ peaks,
-                                                                   int64_t* __restrict__ count,
-                                                                   int32_t* __restrict__ chunk_count,
-                                                                   int32_t* __restrict__ list /* [2][n_items] */,
-                                                                   unsigned long long* __restrict__ list_n /* [2] */) {
-  const int64_t item = (int64_t)blockIdx.x * kFitWarps + (threadIdx.x >> 5);
+__global__ void __launch_bounds__(kFitCountThreads) fit_count_kernel(int64_t n_items, int top_k,
+                                                                    const int64_t* __restrict__ row_ptr,
+                                                                    const double* __restrict__ t,
+                                                                    const qlp_bls_peak* __restrict__ peaks,
+                                                                    int64_t* __restrict__ count,
+                                                                    int32_t* __restrict__ chunk_count,
+                                                                    int32_t* __restrict__ list /* [2][n_items] */,
+                                                                    unsigned long long* __restrict__ list_n /* [2] */) {
+  // one CTA per (star, peak): a 13-sector star has 1.5e5 points, too many for the one warp of round 1
+  const int64_t item = blockIdx.x;
   if (item >= n_items) return;
+  __shared__ int cnt8[kFitCluster];
+  if (threadIdx.x < kFitCluster) cnt8[threadIdx.x] = 0;
+  __syncthreads();
   const int lane = threadIdx.x & 31;
   const int64_t s = item / top_k;
   const qlp_bls_peak pk = peaks[item];
   const FitWindow w = fit_window(pk);
   const int64_t a = row_ptr[s], n = w.valid ? row_ptr[s + 1] - a : 0;
-  int64_t total = 0;
   for (int r = 0; r < kFitCluster; ++r) {
     const int64_t b = fit_chunk_begin(n, r), e = fit_chunk_begin(n, r + 1);
     int c = 0;
 #pragma unroll 4
-    for (int64_t i = b + lane; i < e; i += 32) c += fabs(fit_dt(t[a + i], w)) <= w.win ? 1 : 0;
+    for (int64_t i = b + threadIdx.x; i < e; i += kFitCountThreads) c += fabs(fit_dt(t[a + i], w)) <= w.win ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    if (lane == 0) chunk_count[item * kFitCluster + r] = c;
-    total += c;
+    if (lane == 0 && c) atomicAdd(&cnt8[r], c);
   }
-  if (lane == 0) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int64_t total = 0;
+    for (int r = 0; r < kFitCluster; ++r) { chunk_count[item * kFitCluster + r] = cnt8[r]; total += cnt8[r]; }
     count[item] = total;
     // size class of the fit: 0 = one CTA (also the items without a valid peak), 1 = one cluster
     const int cls = total > kFitSingleMax ? 1 : 0;
