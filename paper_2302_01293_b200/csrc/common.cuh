@@ -144,6 +144,9 @@ __host__ __device__ __forceinline__ int class_nbcap(int c) {
   return caps[c];
 }
 __host__ __device__ __forceinline__ int class_ctas_per_sm(int c) { return c == 0 ? 2 : 1; }
+#ifndef QLP_PAIRED_CLASSES
+#define QLP_PAIRED_CLASSES 1   /* the 32-column class folds two points per warp, 2 columns per lane (foldscan.cuh) */
+#endif
 constexpr int kChunk = 512;                                   // points per staged chunk
 constexpr int kStageBytes = 2 * kChunk * 16 + 16;             // two buffers + two mbarriers
 __host__ __device__ __forceinline__ int class_smem_bytes(int c) {

@@ -162,7 +162,20 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
   __shared__ TileInfo ti;
   __shared__ int64_t s_tile;
   constexpr int STRIDE = 2 * CTOT;              // words per histogram row: [W x CTOT][S x CTOT]
-  constexpr int CW = CTOT < 32 ? CTOT : 32;     // distinct columns across the lanes of a warp
+  // Lane layout of the fold.  128 and 64 columns: the 32 lanes own 4 resp. 2 columns each and fold the same point.
+  // 32 columns ("paired"): a half-warp owns the columns (2 per lane) and the two half-warps fold two different
+  // points, so a point load (2 shared-memory wavefronts whether the lanes read one or two points) feeds 2
+  // evaluations per lane instead of 1.  The two half-warps must not meet on a bank: the second one walks its columns
+  // in the order r ^ 1, so in every instruction the halves work on columns whose indices differ in bit 4 -- the other
+  // half of the banks -- with the same immediate offsets as the wide layouts (measured on config 5: class 3 0.374 ->
+  // 0.415 of the peak; the same layout with 4 columns per lane in the 64-column class: 0.506 -> 0.494, not used).
+  // 16 columns ("quad"): a quarter-warp owns the columns (2 per lane), four points per warp; quarter-warps 1 and 3 walk
+  // their columns in the order r ^ 1 and quarter-warps 2 and 3 add S before W, so the four of them use the four
+  // quarters of the banks (W and S words of columns 0-7 and 8-15) in every instruction.
+  // 8 columns and fewer: one column per lane, 32 / CTOT points per warp, odd point-lanes add S before W.
+  constexpr bool PAIRED = QLP_PAIRED_CLASSES && CTOT == 32;
+  constexpr bool QUAD = QLP_PAIRED_CLASSES && CTOT == 16;
+  constexpr int CW = QUAD ? 8 : (CTOT < 32 ? CTOT : (PAIRED ? 16 : 32));   // distinct columns across the lanes of a warp
   constexpr int R = CTOT / CW;                  // columns per lane
   constexpr int HPW = 32 / CW;                  // points per warp iteration
   constexpr int STEP = kWarps * HPW;            // points consumed per iteration by the CTA
@@ -253,9 +266,12 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       // (never scanned) column: cheaper than predicating every atomic.
       double f[R], dnb[R];
       uint32_t neg_nb_row[R];  // -(nb * row bytes) mod 2^32
+      uint32_t lane_off[R];    // byte offset of the lane's r-th column in a histogram row; where the columns of a
+                               // lane are CW apart in a fixed order it is lane_off[0] + an immediate
 #pragma unroll
       for (int r = 0; r < R; ++r) {
-        const int col = col0 + 32 * r;
+        const int col = col0 + CW * ((PAIRED || QUAD) ? (r ^ (hsub & 1)) : r);
+        lane_off[r] = (uint32_t)((PAIRED || QUAD) ? col : col0) * 4u;
         f[r] = 0.0;
         int32_t nbk = 1;
         if (col < ti.ncols) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
@@ -265,9 +281,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const int64_t n = ti.n_pts;
       const Point* src = pts + ti.pt_begin;
       const int64_t n_chunks = (n + kChunk - 1) / kChunk;
-      const bool swap_ws = (HPW > 1) && (hsub & 1);
+      const bool swap_ws = (HPW > 1) && !PAIRED && (QUAD ? (hsub & 2) != 0 : (hsub & 1) != 0);
       const int first_off = swap_ws ? CTOT : 0;
-      const uint32_t lane_off = (uint32_t)col0 * 4u;  // byte offset of this lane's first column in a row
       unsigned char* hbytes = reinterpret_cast<unsigned char*>(hist);
       __syncthreads();  // histograms zeroed
       clk1s = phase ? clock64() : 0;
@@ -299,13 +314,14 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
               // byte offset of the bin's row: (I - nb g) * row bytes, as I * row + g * (-nb row) (+ lane)
               uint32_t I, g;
               bin_parts(f[r], tau, dnb[r], I, g);
-              const uint32_t off = g * neg_nb_row[r] + (I * (uint32_t)(STRIDE * 4) + lane_off);
-              uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + 32 * r;
-              // check build: the row of the cell lies inside this tile's histogram (bin < nb of the column <= nb_tile)
+              const uint32_t off = g * neg_nb_row[r] + (I * (uint32_t)(STRIDE * 4) + lane_off[r]);
+              uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + ((PAIRED || QUAD) ? 0 : CW * r);
+              // check build: the cell lies inside this tile's histogram (bin < nb of the column <= nb_tile)
               if (!QLP_IN_BOUNDS(kChkFoldCell, off / (uint32_t)(STRIDE * 4) < (uint32_t)nb_tile &&
-                                                   (off % (uint32_t)(STRIDE * 4)) / 4u + 32u * r < (uint32_t)CTOT))
+                                                   (off % (uint32_t)(STRIDE * 4)) / 4u + (uint32_t)((PAIRED || QUAD) ? 0 : CW * r) <
+                                                       (uint32_t)CTOT))
                 continue;
-              if (HPW == 1) {
+              if (HPW == 1 || PAIRED) {
                 atomicAdd(cell, (uint32_t)v[u].z);
                 atomicAdd(cell + CTOT, (uint32_t)v[u].w);
               } else {
@@ -349,7 +365,8 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
       const int per = (nbk + TPC - 1) / TPC;
       const int ja = seg * per;
       const int jb = min(nbk, ja + per);
-      const uint32_t* hc = hist + scol;
+      const uint32_t* hc = hist + scol;                                  // W words of this column
+      const uint32_t* hs = hist + CTOT + scol;                           // S words of this column
       const float inv_w = ti.inv_w;
       const uint32_t wmask = WM ? WM : prm.wmask;
       if (ja < jb) {
@@ -360,7 +377,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
           int e = ja + l;
           if (e >= nbk) e -= nbk;
           ww[l] = (float)hc[e * STRIDE] * inv_w;
-          ss[l] = (float)(int32_t)hc[e * STRIDE + CTOT];
+          ss[l] = (float)(int32_t)hs[e * STRIDE];
         }
         ww[MW - 1] = 0.f; ss[MW - 1] = 0.f;
         for (int j0 = ja; j0 < jb; j0 += MW) {
@@ -372,7 +389,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
               if (e >= nbk) e -= nbk;
               if (!QLP_IN_BOUNDS(kChkScanBin, e >= 0 && e < nbk && nbk <= nb_tile)) e = 0;
               ww[(jj + MW - 1) % MW] = (float)hc[e * STRIDE] * inv_w;
-              ss[(jj + MW - 1) % MW] = (float)(int32_t)hc[e * STRIDE + CTOT];
+              ss[(jj + MW - 1) % MW] = (float)(int32_t)hs[e * STRIDE];
               float r = 0.f, sm = 0.f, vj = 0.f;
 #pragma unroll
               for (int m = 1; m <= MW; ++m) {
@@ -408,6 +425,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         bj = (int)(bidx & 0xffffffu);
         {
           const uint32_t* hcw = hist + scol;
+          const uint32_t* hsw = hist + CTOT + scol;
           const uint32_t wmask = WM ? WM : prm.wmask;
           float r = 0.f, sm = 0.f;
           bm = 0;
@@ -416,7 +434,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
             int e = bj + m - 1;
             if (e >= nbk) e -= nbk;
             r = __fadd_rn(r, (float)hcw[e * STRIDE] * ti.inv_w);
-            sm = __fadd_rn(sm, (float)(int32_t)hcw[e * STRIDE + CTOT]);
+            sm = __fadd_rn(sm, (float)(int32_t)hsw[e * STRIDE]);
             if (((wmask >> m) & 1u) && bm == 0 && box_value(r, sm) == bval) bm = m;
           }
         }
@@ -425,10 +443,11 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         // take the narrowest ladder width that still covers the occupied span and, for it, the
         // smallest start bin whose extra bins are all empty.
         const uint32_t* hc = hist + scol;
+        const uint32_t* hs2 = hist + CTOT + scol;
         // a bin is empty only if both words are zero (a point of tiny weight may quantise to W = 0 with S != 0)
         auto empty = [&](int e) {
           e %= nbk; if (e < 0) e += nbk;
-          return (hc[e * STRIDE] | hc[e * STRIDE + CTOT]) == 0u;
+          return (hc[e * STRIDE] | hs2[e * STRIDE]) == 0u;
         };
         int a = bj, b = bj + bm - 1;
         while (a < b && empty(a)) ++a;
