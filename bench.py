@@ -243,6 +243,8 @@ class OracleSample:
         per_thread = rate / max(min(threads, med.size), 1)
         ok = np.nonzero((cost > 0) & (cost <= 0.5 * budget_s * per_thread))[0]
         ok = ok[np.argsort(cost[ok], kind="stable")]
+        if ok.size == 0:   # a budget below one star per thread: the cheapest stars, one per thread
+            ok = np.argsort(np.where(cost > 0, cost, np.inf), kind="stable")[:max(1, min(threads, int((cost > 0).sum())))]
         want = 0.7 * budget_s * rate
         n_light = int(max(min(ok.size, threads), min(ok.size, want / max(cost[ok].mean(), 1.0)))) if ok.size else 0
         pick = np.unique(ok[np.linspace(0, ok.size - 1, n_light).round().astype(np.int64)]) if n_light else ok[:0]

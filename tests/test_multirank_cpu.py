@@ -152,3 +152,30 @@ def test_parallel_generation_reproduces_make_batch():
     for k in ("row_ptr", "t", "y", "dy", "rho"):
         assert np.array_equal(getattr(got2, k), getattr(ref2, k)), k
     assert np.array_equal(rp, ref2.row_ptr) and np.array_equal(t, ref2.t) and np.array_equal(rho, ref2.rho)
+
+
+def test_gather_without_a_process_group_is_a_reorder():
+    """One GPU: no process group; the gathered table is the local one put in global star order."""
+    from paper_2302_01293_b200 import shard
+    ids = np.array([3, 0, 2, 1])
+    got = shard.gather_tables(_fake_peak_table(ids), ids, 4)
+    assert got.tobytes() == _fake_peak_table(np.arange(4)).tobytes()
+    with pytest.raises(RuntimeError):                       # rows that do not partition the job are refused
+        shard.unpack_rows(shard.pack_rows(_fake_peak_table(np.array([0, 0])), np.array([0, 0])), 2,
+                          _fake_peak_table(ids).dtype, (3,))
+
+
+def test_reference_arm_prints_one_json_line(capsys):
+    """bench.py --impl reference on rank 0: one JSON line with the contract's keys, timed on a bounded oracle sample."""
+    import json
+    import bench
+    args = type("A", (), {"stars": 12, "config": 2, "steps": 1, "warmup": 0, "gpus": 1, "ref_budget": 0.3})()
+    bench.run_reference(args)
+    lines = [ln for ln in capsys.readouterr().out.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == bench.METRIC and d["unit"] == bench.UNIT
+    assert d["value"] > 0 and d["higher_is_better"] is True and d["vs_baseline"] is None
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"] == {"value": d["value"], "unit": bench.UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "workload" in d["config"] and d["gpu_launches"] == 0
