@@ -181,3 +181,35 @@ def test_star_above_point_cap_is_skipped(gpu):
         assert pk[0][0]["k"] == -1 and pk[1][0]["k"] >= 0
     finally:
         ctx.close()
+
+
+def test_tile_classes_cover_every_star_and_frequency_once(gpu):
+    """The per-class work counters of the fold/scan kernel (qlp_bls_fold_class_counters, what bench.py's roofline
+    entry is built from): over a ragged production-shaped batch the evaluations of all tile classes add up to
+    sum_s N_s n_freq,s exactly -- every (star, frequency) is folded once, by one tile of one class."""
+    from paper_2302_01293_b200 import synth
+    b = synth.make_batch(5, star_ids=np.arange(80))
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        dev = gpu.upload(b)
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        g = gpu.grid_to_numpy(grid)
+        ctx.fold_timing(True)
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        cc = ctx.fold_class_counters()
+        n_timed, ms = ctx.fold_elapsed_ms()
+        ctx.fold_timing(False)
+        want = int((g["n_freq"].astype(np.int64) * np.diff(b.row_ptr)).sum())
+        assert int(cc[:, 3].sum()) == want
+        assert n_timed == 1 and ms > 0.0
+        assert int((cc[:, 4] > 0).sum()) >= 4                      # several tile classes are populated
+        assert np.all(cc[cc[:, 4] == 0][:, :4] == 0)               # a class without tiles did no work
+        # the trapezoid fits count their work too while timing is on
+        _, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best, want_snr=False)
+        ctx.fold_timing(True)
+        fits = gpu.fits_to_numpy(ctx.trapezoid_fit(dev[0], dev[1], dev[2], dev[3], peaks), ctx.top_k)
+        pairs = ctx.fit_work()
+        ctx.fold_timing(False)
+        assert pairs > 0 and pairs <= int((fits["n_fit"].astype(np.int64) * fits["n_eval"]).sum())
+    finally:
+        ctx.close()
