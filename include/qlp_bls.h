@@ -23,6 +23,9 @@
  *     [row_ptr[s], row_ptr[s+1]).  Frequencies: freq_ptr[S+1] (int64), ascending frequency within
  *     a star.  t in days (any zero point), strictly increasing within a star; y any linear flux
  *     unit; dy > 0.  rho in solar units (non-finite or <= 0 means "solar").
+ *     The weights dy^-2 / sum dy^-2 are accumulated in 32-bit fixed point (resolution 2^-32 of a star's total
+ *     weight): the SR tolerance of 1e-4 of the peak holds for errors that vary by less than a factor ~30 within one
+ *     light curve; beyond that, boxes made of a few very light points are resolved to a few 1e-4.
  */
 #ifndef QLP_BLS_H_
 #define QLP_BLS_H_
