@@ -132,3 +132,44 @@ def test_trapezoid_fit_empty_and_invalid(gpu):
         assert ctx.trapezoid_fit(empty, empty.double(), empty.double(), empty.double(), empty).numel() == 0
     finally:
         ctx.close()
+
+
+def test_trapezoid_fit_on_random_irregular_stars(gpu, orc):
+    """The fit, the statistics and the noise row on 60 random irregular stars (exponential spacings, gaps, outliers,
+    5 to 4,000 points: windows of a handful of points, q at its bounds, peaks without a fit) against the oracle:
+    the same strict comparison as above on every fit."""
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(777)
+    stars, rho = [], []
+    for i in range(60):
+        n = int(rng.integers(5, 4000))
+        dt = rng.exponential(rng.choice([200.0, 600.0, 1800.0]) / 86400.0, n) + 1e-5
+        for _ in range(int(rng.integers(0, 3))):
+            dt[int(rng.integers(0, n))] += rng.choice([0.7, 3.0, 29.0])
+        t = 2000.0 + np.cumsum(dt)
+        dy = 1e-3 * 10.0 ** rng.uniform(-0.3, 0.3, n)
+        y = rng.standard_normal(n) * dy + 1.0
+        if i % 3 == 0:
+            p = rng.uniform(0.4, 5.0)
+            y -= rng.uniform(2e-3, 1e-2) * (np.mod(t - t[0], p) < 0.04 * p)
+        stars.append((t, y, dy))
+        rho.append(10.0 ** rng.uniform(-1.0, 1.0))
+    b = synth.from_arrays(stars, rho=np.array(rho))
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        pk, fits = run_search(gpu, ctx, b)
+        dev = gpu.upload(b)
+        checked = 0
+        for s in range(b.n_stars):
+            t, y, dy = b.star(s)
+            for r in range(ctx.top_k):
+                p, g = pk[s][r], fits[s][r]
+                if p["k"] < 0:
+                    assert g["status"] == 1 and g["n_fit"] == 0
+                    continue
+                o = orc.trapezoid_fit(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]))
+                compare(orc, (t, y, dy), g, o, p)
+                checked += 1
+        assert checked > 120
+    finally:
+        ctx.close()

@@ -127,3 +127,55 @@ def test_pink_noise_empty_and_invalid(gpu):
             assert pink[1][r]["sigma_w"] == 0.0 and pink[1][r]["snr_pink"] == 0.0 and pink[1][r]["detected"] == 0
     finally:
         ctx.close()
+
+
+def test_statistics_and_noise_row_on_random_irregular_stars(gpu, orc):
+    """O7 and O9 on 60 random irregular stars (exponential spacings, gaps, outliers, 5 to 4,000 points): counts
+    bit-exact, noise estimates and S/N_pink at the tolerances above, on every peak that has a fit."""
+    from paper_2302_01293_b200 import synth
+    rng = np.random.default_rng(4242)
+    stars, rho = [], []
+    for i in range(60):
+        n = int(rng.integers(5, 4000))
+        dt = rng.exponential(rng.choice([200.0, 600.0, 1800.0]) / 86400.0, n) + 1e-5
+        for _ in range(int(rng.integers(0, 3))):
+            dt[int(rng.integers(0, n))] += rng.choice([0.7, 3.0, 29.0])
+        t = 2000.0 + np.cumsum(dt)
+        dy = 1e-3 * 10.0 ** rng.uniform(-0.3, 0.3, n)
+        y = rng.standard_normal(n) * dy + 1.0
+        if i % 3 == 0:
+            p = rng.uniform(0.4, 5.0)
+            y -= rng.uniform(2e-3, 1e-2) * (np.mod(t - t[0], p) < 0.04 * p)
+        stars.append((t, y, dy))
+        rho.append(10.0 ** rng.uniform(-1.0, 1.0))
+    b = synth.from_arrays(stars, rho=np.array(rho))
+    ctx = gpu.QlpBls(top_k=3)
+    try:
+        pk, fits, pink = run(gpu, ctx, b)
+        dev = gpu.upload(b)
+        # run() made its own device copies; the statistics need the peak table on the device again
+        grid, fp, tf, _ = ctx.grid(dev[0], dev[1], dev[4], dev[5])
+        sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, fp, tf)
+        _, peaks = ctx.snr(dev[0], dev[1], dev[2], dev[3], grid, fp, sr, best, want_snr=False)
+        assert gpu.peaks_to_numpy(peaks, ctx.top_k).tobytes() == pk.tobytes()       # bitwise reproducible
+        stats = gpu.stats_to_numpy(ctx.peak_stats(dev[0], dev[1], dev[2], dev[3], peaks), ctx.top_k)
+        n_pink = n_stats = 0
+        for s in range(b.n_stars):
+            t, y, dy = b.star(s)
+            for r in range(ctx.top_k):
+                p, ft, g, st = pk[s][r], fits[s][r], pink[s][r], stats[s][r]
+                if p["k"] < 0:
+                    continue
+                o = orc.peak_statistics(t, y, dy, float(p["freq"]), int(p["m"]), int(p["nb"]), float(p["t0"]))
+                for k in ("n_in", "n_before", "n_after", "n_transits"):
+                    assert st[k] == o[k], (s, r, k, st[k], o[k])
+                assert abs(st["oot_level"] - o["oot_level"]) <= 1e-12 * max(1.0, abs(o["oot_level"]))
+                n_stats += 1
+                if ft["status"] != 0:
+                    assert g.tobytes() == bytes(48)
+                    continue
+                compare(orc, (t, y, dy), p, ft, g)
+                n_pink += 1
+        assert n_stats > 120 and n_pink > 100
+    finally:
+        ctx.close()
