@@ -433,18 +433,33 @@ def test_random_irregular_stars(gpu, ctx, orc, cfg):
 def test_weight_dynamic_range_limit(gpu, ctx, orc, cfg):
     """The documented limit of the fixed-point weights (W_i = round(w_i 2^32)): with errors
     spread over two decades (weights over four) a box can consist of a few points that each carry < 1e-6 of the
-    total weight, and its r is then quantised to a few 1e-4.  The spectrum stays within 1e-3 of the peak (ten times
-    the tolerance that holds for every realistic weight range) and nothing else degrades: grid bit-exact, S/N finite."""
+    total weight, and its r is then quantised to a few 1e-4.  The star below is the one on which the fuzz test first
+    ran into it (the 114th star of the same random stream with two decades of errors: 3,412 points, best box of
+    one frequency holds r = 8e-7): the spectrum leaves the 1e-4 tolerance by a hair and stays within 1e-3 of the
+    peak; nothing else degrades (grid bit-exact, S/N finite)."""
     from paper_2302_01293_b200 import synth
-    rng = np.random.default_rng(113)
-    n = 3400
-    t = 2000.0 + np.cumsum(rng.exponential(600.0 / 86400.0, n) + 1e-5)
-    dy = 1e-3 * 10.0 ** rng.uniform(-1.0, 1.0, n)
-    y = rng.standard_normal(n) * dy + 1.0
-    b = synth.from_arrays([(t, y, dy)], rho=np.array([20.0]))
+    rng = np.random.default_rng(2024)
+    for i in range(114):
+        n = int(rng.integers(5, 4000))
+        dt = rng.exponential(rng.choice([200.0, 600.0, 1800.0]) / 86400.0, n) + 1e-5
+        for _ in range(int(rng.integers(0, 4))):
+            dt[int(rng.integers(0, n))] += rng.choice([0.7, 3.0, 29.0, 45.0])
+        t = 2000.0 + np.cumsum(dt)
+        dy = 1e-3 * 10.0 ** rng.uniform(-1.0, 1.0, n)
+        y = rng.standard_normal(n) * dy + 1.0
+        if i % 5 == 0:
+            y[rng.integers(0, n, max(1, n // 100))] += 0.05
+        if i % 7 == 0:
+            p = rng.uniform(0.4, 5.0)
+            y -= 5e-3 * (np.mod(t - t[0], p) < 0.05 * p)
+        rho = 10.0 ** rng.uniform(-1.5, 1.5)
+    assert n == 3412
+    b = synth.from_arrays([(t, y, dy)], rho=np.array([rho]))
     res = _search(gpu, ctx, b, want_snr=True)
     ob = orc.batch(cfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=0, want_snr=False)
     assert res["grid"].tobytes() == ob["grid"].tobytes()
+    w = dy ** -2.0 / np.sum(dy ** -2.0)
+    assert w.min() < 1e-6 and w.max() / w.min() > 5e3
     err = np.abs(res["sr"].astype(np.float64) - ob["sr"]).max() / ob["sr"].max()
-    print(f"weights over four decades: worst |dSR|/peak = {err:.2e}")
-    assert err <= 1e-3 and np.all(np.isfinite(res["snr"]))
+    print(f"weights over four decades (lightest point {w.min():.1e} of the total): worst |dSR|/peak = {err:.2e}")
+    assert 5e-5 < err <= 1e-3 and np.all(np.isfinite(res["snr"]))
