@@ -15,6 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "qlp_oracle.c")
 _LIB = os.path.join(_HERE, "libqlp_oracle.so")
+_LIB_SAN = os.path.join(_HERE, "libqlp_oracle_san.so")
 
 
 class Config(C.Structure):
@@ -44,8 +45,21 @@ def default_config(**kw) -> Config:
     return c
 
 
+def sanitized() -> bool:
+    """QLP_ORACLE_SANITIZE=1: the same source built with AddressSanitizer + UndefinedBehaviorSanitizer (any report
+    aborts).  The process must have libasan preloaded (tests/test_oracle_sanitized.py starts such a child)."""
+    return os.environ.get("QLP_ORACLE_SANITIZE", "0") == "1"
+
+
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (FP64, no FMA contraction, OpenMP over stars)."""
+    if sanitized():
+        if force or not os.path.exists(_LIB_SAN) or os.path.getmtime(_LIB_SAN) < os.path.getmtime(_SRC):
+            cmd = ["gcc", "-O1", "-g", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
+                   "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer",
+                   "-std=c11", "-o", _LIB_SAN, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+        return _LIB_SAN
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
                "-std=c11", "-o", _LIB, _SRC, "-lm"]

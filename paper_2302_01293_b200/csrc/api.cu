@@ -7,6 +7,8 @@
 
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>  // header-only; a no-op unless a profiler injects itself (nsys, ncu --nvtx)
+
 #include "common.cuh"
 #include "foldscan.cuh"
 #include "grid.cuh"
@@ -20,6 +22,15 @@ using namespace qlp;
 
 static constexpr int kClassCtr = 8;  // uint64 counters per tile class (5 used), see qlp_bls_fold_class_counters
 static constexpr uint32_t kPaperMask = 0xFF8u;  // widths 3..11 (PAPER.md:19, :35 -> DESIGN.md O1.9)
+
+// One NVTX range per C-ABI call (and per sub-batch of the host driver), named after the call: a timeline lines the
+// stages up with the kernels they launch, and `ncu --nvtx --nvtx-include "qlp_bls_spectrum/"` picks one stage.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+  NvtxRange(const NvtxRange&) = delete;
+  NvtxRange& operator=(const NvtxRange&) = delete;
+};
 
 struct DevBuf {
   void* p = nullptr;
@@ -325,6 +336,7 @@ static int run_validation(qlp_bls_ctx* ctx, int which, int64_t n_stars, const in
 extern "C" int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                             const double* rho, const double* rstar, qlp_bls_star_grid* grid, int64_t* freq_ptr,
                             int64_t* total_freq, int64_t* total_bins, void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_grid");
   (void)rstar;  // R* cancels out of a/R* = (G rho P^2 / 3 pi)^(1/3): DESIGN.md reading A8
   if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr || !total_freq || !total_bins) return QLP_BLS_EINVAL;
   if (n_stars > 0 && (!t || !rho || !grid)) return QLP_BLS_EINVAL;
@@ -393,6 +405,7 @@ static int ensure_side_streams(qlp_bls_ctx* ctx) {
 extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                 const double* y, const double* dy, const qlp_bls_star_grid* grid,
                                 const int64_t* freq_ptr, float* sr, uint32_t* best, void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_spectrum");
   if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr) return QLP_BLS_EINVAL;
   if (n_stars == 0) return QLP_BLS_OK;
   if (!t || !y || !dy || !grid || !sr || !best) return QLP_BLS_EINVAL;
@@ -462,6 +475,7 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
 extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t, const double* y,
                            const double* dy, const qlp_bls_star_grid* grid, const int64_t* freq_ptr, const float* sr,
                            const uint32_t* best, float* snr, qlp_bls_peak* peaks, void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_snr");
   if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr) return QLP_BLS_EINVAL;
   if (n_stars == 0) return QLP_BLS_OK;
   if (!t || !y || !dy || !grid || !sr || !best || !peaks) return QLP_BLS_EINVAL;
@@ -486,6 +500,7 @@ extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row
 extern "C" int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                   const double* y, const double* dy, const qlp_bls_peak* peaks,
                                   qlp_bls_transit_stats* stats, void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_peak_stats");
   if (!ctx || n_stars < 0) return QLP_BLS_EINVAL;
   if (n_stars == 0) return QLP_BLS_OK;
   if (!row_ptr || !t || !y || !dy || !peaks || !stats) return QLP_BLS_EINVAL;
@@ -500,6 +515,7 @@ extern "C" int qlp_bls_peak_stats(qlp_bls_ctx* ctx, int64_t n_stars, const int64
 extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                      const double* y, const double* dy, const qlp_bls_peak* peaks,
                                      qlp_bls_trapezoid* fits, void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_trapezoid_fit");
   if (!ctx || n_stars < 0) return QLP_BLS_EINVAL;
   if (n_stars == 0) return QLP_BLS_OK;
   if (!row_ptr || !t || !y || !dy || !peaks || !fits) return QLP_BLS_EINVAL;
@@ -571,6 +587,7 @@ extern "C" int qlp_bls_trapezoid_fit(qlp_bls_ctx* ctx, int64_t n_stars, const in
 extern "C" int qlp_bls_pink_noise(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                                   const double* y, const qlp_bls_peak* peaks, const qlp_bls_trapezoid* fits,
                                   qlp_bls_pink* pink, void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_pink_noise");
   if (!ctx || n_stars < 0) return QLP_BLS_EINVAL;
   if (n_stars == 0) return QLP_BLS_OK;
   if (!row_ptr || !t || !y || !peaks || !fits || !pink) return QLP_BLS_EINVAL;
@@ -697,6 +714,7 @@ static int search_host_impl(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* ro
     const double* d_y = (const double*)ctx->h_y[set].p;
     const double* d_dy = (const double*)ctx->h_dy[set].p;
     int64_t tf = 0, tb = 0;
+    NvtxRange nvtx_range("qlp_bls_host_sub_batch");
     ctx->prep_valid = false;  // staging pointers are reused across sub-batches: the records are another sub-batch's
     rc = qlp_bls_grid(ctx, S, d_row, d_t, (const double*)ctx->h_rho[set].p, nullptr,
                       (qlp_bls_star_grid*)ctx->h_grid.p, (int64_t*)ctx->h_fptr.p, &tf, &tb, st);
