@@ -44,7 +44,8 @@ enum qlp_bls_status {
   QLP_BLS_ENOMEM = -2,       /* workspace allocation failed                                      */
   QLP_BLS_ECUDA = -3,        /* a CUDA runtime call or kernel launch failed                      */
   QLP_BLS_EUNSUPPORTED = -4, /* e.g. a star needs more phase bins than QLP_BLS_MAX_NB            */
-  QLP_BLS_EVALIDATION = -5   /* flags bit0 set and an input failed validation                    */
+  QLP_BLS_EVALIDATION = -5,  /* flags bit0 set and an input failed validation                    */
+  QLP_BLS_ETOOLARGE = -6     /* qlp_bls_grid_noalloc: n_stars > QLP_BLS_NOALLOC_MAX_STARS        */
 };
 
 /* Largest number of fine phase bins per frequency (two FP32 histograms of one frequency must fit
@@ -185,6 +186,30 @@ int qlp_bls_create(const qlp_bls_config* cfg /*host*/, qlp_bls_ctx** out /*host*
 int qlp_bls_grid(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
                  const double* rho, const double* rstar, qlp_bls_star_grid* grid, int64_t* freq_ptr,
                  int64_t* total_freq, int64_t* total_bins, void* cuda_stream);
+
+/* S1 for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same two kernels as qlp_bls_grid (O1), same grid
+ * descriptors and freq_ptr bit for bit, but the stage's scratch array (one 64-bit sum of nb_k per star) is a
+ * file-scope __device__ array of the library instead of context workspace, and the two totals stay on the device.
+ * The call makes no cudaMalloc / cudaFree / allocating library call, copies nothing to the host and does not
+ * synchronise: it enqueues one memset of the used scratch prefix and two kernels on `cuda_stream`.
+ *   in : row_ptr dev int64[S+1]; t dev double[row_ptr[S]]; rho dev double[S]
+ *   out: grid dev [S]; freq_ptr dev int64[S+1]; totals dev int64[2] = { freq_ptr[S], sum of nb_k }.
+ * Limits and contract:
+ *   - n_stars <= QLP_BLS_NOALLOC_MAX_STARS (262,144; the static array is 2 MiB, held by every GPU that loads the
+ *     library until the process exits); a larger batch returns QLP_BLS_ETOOLARGE and enqueues nothing;
+ *   - no input validation pass, whatever flags bit0 says (it needs a read-back); stars with non-increasing or
+ *     non-finite timestamps still get status 7 and n_freq = 0 as in qlp_bls_grid;
+ *   - ALL calls on a device share the one array, and it keeps the last call's contents: two calls that may overlap
+ *     on the GPU (different streams, different contexts, different host threads) race on it.  Serialise them
+ *     (one stream, or an event between them);
+ *   - the first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device): make
+ *     one call before starting a graph capture.
+ * `ctx` supplies the search parameters and the device; its workspace is not touched. */
+#define QLP_BLS_NOALLOC_MAX_STARS 262144
+int qlp_bls_grid_noalloc(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                         const double* rho, qlp_bls_star_grid* grid, int64_t* freq_ptr, int64_t* totals,
+                         void* cuda_stream);
 
 /* S0 + S2 + S3: weights and centred series (Kovacs 2002 weighting), fold-and-bin
  * at every grid frequency, box scan over every start bin and every width of the duration ladder

@@ -46,7 +46,7 @@ TRAP_DTYPE = np.dtype([("t0", "f8"), ("depth", "f8"), ("q", "f8"), ("q_in", "f8"
 PINK_DTYPE = np.dtype([("sigma_w", "f8"), ("sigma_r", "f8"), ("depth_eff", "f8"), ("snr_pink", "f8"),
                        ("n_t", "i4"), ("n_transits", "i4"), ("n_bins", "i4"), ("detected", "i4")], align=True)
 
-EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_vet_host", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_spectrum", "qlp_bls_snr",
+EXPORTS = ["qlp_bls_peak_stats", "qlp_bls_trapezoid_fit", "qlp_bls_pink_noise", "qlp_bls_vet_host", "qlp_bls_default_config", "qlp_bls_create", "qlp_bls_grid", "qlp_bls_grid_noalloc", "qlp_bls_spectrum", "qlp_bls_snr",
            "qlp_bls_search_host", "qlp_bls_destroy", "qlp_bls_strerror", "qlp_bls_launch_count",
            "qlp_bls_widths", "qlp_bls_fold_timing", "qlp_bls_fold_elapsed_ms", "qlp_bls_fold_phase_clocks", "qlp_bls_fold_class_counters", "qlp_bls_fit_work", "qlp_bls_debug_freqs", "qlp_bls_debug_bins", "qlp_bls_debug_prep",
            "qlp_bls_debug_set_path", "qlp_bls_debug_violations"]
@@ -68,6 +68,7 @@ def load_library(check: bool = False):
         L.qlp_bls_default_config.restype = None
         L.qlp_bls_create.argtypes = [C.POINTER(Config), C.POINTER(vp)]
         L.qlp_bls_grid.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64), C.POINTER(i64), vp]
+        L.qlp_bls_grid_noalloc.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_spectrum.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_snr.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.qlp_bls_peak_stats.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
@@ -205,6 +206,13 @@ class QlpBls:
         _check(self.lib.qlp_bls_grid(self._h, S, _ptr(row_ptr), _ptr(t), _ptr(rho), _ptr(rstar), _ptr(grid),
                                      _ptr(freq_ptr), C.byref(tf), C.byref(tb), self._stream()), "qlp_bls_grid")
         return grid, freq_ptr, int(tf.value), int(tb.value)
+
+    def grid_noalloc(self, row_ptr, t, rho, grid, freq_ptr, totals):
+        """qlp_bls_grid_noalloc: S1 into caller-provided device tensors (grid uint8[S, 72], freq_ptr int64[S+1],
+        totals int64[2]); the library allocates nothing, copies nothing back and does not synchronise."""
+        S = int(row_ptr.numel()) - 1
+        _check(self.lib.qlp_bls_grid_noalloc(self._h, S, _ptr(row_ptr), _ptr(t), _ptr(rho), _ptr(grid),
+                                             _ptr(freq_ptr), _ptr(totals), self._stream()), "qlp_bls_grid_noalloc")
 
     # -- S0 + S2 + S3
     def spectrum(self, row_ptr, t, y, dy, grid, freq_ptr, total_freq: int):

@@ -2,6 +2,7 @@
 // Every step of the path runs in the kernels of grid.cuh / prep.cuh / foldscan.cuh / snr_kernel.cuh;
 // the host code below only sizes buffers and enqueues work.
 #include <math.h>
+#include <mutex>
 #include <new>
 #include <string.h>
 
@@ -234,6 +235,7 @@ extern "C" const char* qlp_bls_strerror(int code) {
     case QLP_BLS_ECUDA: return "CUDA error";
     case QLP_BLS_EUNSUPPORTED: return "unsupported";
     case QLP_BLS_EVALIDATION: return "input validation failed";
+    case QLP_BLS_ETOOLARGE: return "batch exceeds the static scratch of the no-allocation entry point";
     default: return "unknown status";
   }
 }
@@ -834,5 +836,54 @@ extern "C" int qlp_bls_debug_prep(qlp_bls_ctx* ctx, const int64_t* row_ptr, cons
   if (ctx->grid_row_ptr != row_ptr || ctx->grid_n_stars <= star) return QLP_BLS_EINVAL;
   QLP_TRY(run_prep(ctx, ctx->grid_n_stars, row_ptr, t, y, dy, grid, st));
   debug_prep_kernel<<<64, 256, 0, st>>>(row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, star, tau, w, wy);
+  return launch_ok(ctx);
+}
+
+// ---- S1 without any allocation --------------------------------------------------------------------------
+// qlp_bls_grid_noalloc: the grid stage (grid_kernel + freq_scan_kernel, the kernels of qlp_bls_grid) for callers that
+// cannot call cudaMalloc.  The one scratch array of the stage -- the per-star sum of nb_k that grid_kernel writes
+// and freq_scan_kernel adds up -- lives in the file-scope device array below instead of the context's workspace.
+// Every GPU that loads the library holds these (QLP_BLS_NOALLOC_MAX_STARS + 1) x 8 bytes = 2 MiB until exit.
+static __device__ __align__(256) unsigned long long g_noalloc_star_bins[QLP_BLS_NOALLOC_MAX_STARS + 1];
+
+// In host code `g_noalloc_star_bins` is only the host-side stand-in of the symbol, not a device address: the
+// address the kernels get is resolved with cudaGetSymbolAddress, once per device, with that device current.
+static constexpr int kNoAllocMaxDevices = 64;
+static unsigned long long* g_noalloc_dev_ptr[kNoAllocMaxDevices] = {};
+static std::mutex g_noalloc_mutex;
+
+static int noalloc_scratch(int device, unsigned long long** out) {
+  if (device < 0 || device >= kNoAllocMaxDevices) return QLP_BLS_EUNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_dev_ptr[device]) {
+    unsigned long long* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_star_bins);   // the current device's copy
+    if (e != cudaSuccess || !p) { cudaGetLastError(); return QLP_BLS_ECUDA; }
+    g_noalloc_dev_ptr[device] = p;
+  }
+  *out = g_noalloc_dev_ptr[device];
+  return 0;
+}
+
+extern "C" int qlp_bls_grid_noalloc(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row_ptr, const double* t,
+                                    const double* rho, qlp_bls_star_grid* grid, int64_t* freq_ptr, int64_t* totals,
+                                    void* cuda_stream) {
+  NvtxRange nvtx_range("qlp_bls_grid_noalloc");
+  if (!ctx || n_stars < 0 || !row_ptr || !freq_ptr || !totals) return QLP_BLS_EINVAL;
+  if (n_stars > 0 && (!t || !rho || !grid)) return QLP_BLS_EINVAL;
+  if (n_stars > (int64_t)QLP_BLS_NOALLOC_MAX_STARS) return QLP_BLS_ETOOLARGE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(ctx->device));
+  unsigned long long* star_bins = nullptr;
+  QLP_TRY(noalloc_scratch(ctx->device, &star_bins));
+  // The array keeps the previous call's contents.  grid_kernel writes every element that freq_scan_kernel reads
+  // (one per star), so nothing has to start at zero; the used prefix is cleared all the same, so that a launch
+  // that fails half-way cannot hand an earlier batch's sums to the scan.
+  CUDA_TRY(cudaMemsetAsync(star_bins, 0, (size_t)(n_stars + 1) * sizeof(unsigned long long), st));
+  if (n_stars > 0) {
+    grid_kernel<<<(unsigned)n_stars, 256, 0, st>>>(ctx->prm, n_stars, row_ptr, t, rho, grid, star_bins);
+    QLP_TRY(launch_ok(ctx));
+  }
+  freq_scan_kernel<<<1, 1024, 0, st>>>(n_stars, grid, star_bins, freq_ptr, totals);
   return launch_ok(ctx);
 }
