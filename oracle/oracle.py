@@ -20,7 +20,7 @@ _LIB_SAN = os.path.join(_HERE, "libqlp_oracle_san.so")
 
 class Config(C.Structure):
     _fields_ = [("samples_per_peak", C.c_double), ("dlogq", C.c_double), ("noverlap", C.c_int32),
-                ("pad_", C.c_int32), ("qmin_fac", C.c_double), ("qmax_fac", C.c_double),
+                ("uniform_freq", C.c_int32), ("qmin_fac", C.c_double), ("qmax_fac", C.c_double),
                 ("a_over_rstar_min", C.c_double), ("sector_days", C.c_double),
                 ("max_period_days", C.c_double), ("max_freq", C.c_int64)]
 

@@ -37,7 +37,7 @@ typedef struct {
   double samples_per_peak; /* 2.0 */
   double dlogq;            /* 0.1 */
   int32_t noverlap;        /* 3 */
-  int32_t pad_;
+  int32_t uniform_freq;    /* 0; 1 = O1.10c, the comparison grid with equal steps in frequency */
   double qmin_fac;         /* 0.5 */
   double qmax_fac;         /* 2.0 */
   double a_over_rstar_min; /* 2.0 (3.0 for Sectors 59-60) */
@@ -49,10 +49,11 @@ typedef struct {
 } orc_config;
 
 typedef struct {
-  double t_ref, baseline, p_min, p_max, c_q, u0, h;
+  double t_ref, baseline, p_min, p_max, c_q, u0, h; /* h > 0: f_k = (u0 + k h)^3; h < 0 (O1.10c): f_k = u0 + k (-h) */
   int64_t n_freq;
   int32_t nb_max;
-  int32_t status; /* 0 ok; 1: fewer than 2 points; 2: baseline <= 0; 3: f_max <= f_min */
+  int32_t status; /* 0 ok; 1: fewer than 2 points; 2: baseline <= 0; 3: f_max <= f_min (or, O1.10c, a frequency
+                     step below 1e-9 f_max) */
 } orc_star_grid;
 
 typedef struct {
@@ -164,11 +165,39 @@ void orc_grid(const orc_config* c, int64_t n, const double* t, double rho_in, or
     double qlo = Q * u2;
     g->nb_max = (int32_t)ceil(((double)c->noverlap) / qlo);
   }
+  /* O1.10c: the comparison grid with equal steps in FREQUENCY (the shape of the earlier CPU search, PAPER.md:13:
+   * "an under-sampled frequency grid on the order of 80,000 frequencies or less"): f_k = f_min + k df over the same
+   * range [f_min, f_max].  df is the step the f^(1/3) law has at f_min, where it is finest (d(u^3)/dk = 3 u^2 h =
+   * A u0^2), so that no part of the range is sampled more coarsely than the GPU grid samples it; when that takes
+   * more than max_freq points the range is under-sampled to exactly max_freq of them.  nb_k keeps the Keplerian
+   * law of O1.8 at f_k.  The descriptor holds u0 = f_min and h = -df: the sign of h marks the grid's kind.
+   * A step below 1e-9 f_max is refused (status 3): cbrt_det is accurate to a few 1e-16, so above that bound
+   * u_k = cbrt_det(f_k) and with it nb_k are monotone in k. */
+  if (c->uniform_freq) {
+    double df = A * (u0 * u0);
+    g->n_freq = (int64_t)floor((f_max - f_min) / df) + 1;
+    if (c->max_freq >= 2 && g->n_freq > c->max_freq) {
+      df = (f_max - f_min) / (double)(c->max_freq - 1);
+      g->n_freq = c->max_freq;
+    }
+    if (!(df > 1e-9 * f_max)) { g->status = 3; g->n_freq = 0; g->nb_max = 0; g->u0 = 0.0; g->h = 0.0; return; }
+    g->u0 = f_min;
+    g->h = -df;
+  }
 }
 
 /* O1.8: frequency k and its number of fine phase bins. */
 void orc_freq(const orc_config* c, const orc_star_grid* g, int64_t k, double* f, int32_t* nb) {
   double Q = c->qmin_fac * g->c_q;
+  if (g->h < 0.0) { /* O1.10c: equal steps in frequency, Keplerian nb at f_k */
+    double fk = g->u0 + ((double)k) * (-g->h);
+    double u = orc_cbrt_det(fk);
+    double u2 = u * u;
+    *f = fk;
+    double qlo = Q * u2;
+    *nb = (int32_t)ceil(((double)c->noverlap) / qlo);
+    return;
+  }
   double u = g->u0 + ((double)k) * g->h;
   double u2 = u * u;
   *f = u2 * u;

@@ -188,6 +188,87 @@ def test_comparison_grid_caps(orc, cfg):
     assert 5.0 < ratio(10.0) < 15.0 and 2.0 < ratio(1.0) < 4.0
 
 
+def test_comparison_grid_uniform_in_frequency(orc, cfg):
+    """O1.10c: the comparison grid with equal steps in frequency.  Pins, none of
+    them the oracle's own formula: the frequencies are an arithmetic progression from 1/P_max to (at most) 1/P_min;
+    uncapped, its step is the smallest step of the GPU grid (the one at its low-frequency end); capped, exactly
+    max_freq points over the same range; nb_k is the Keplerian ceil(noverlap / (0.5 q_circ(f_k))) with q_circ from
+    Kepler's third law in SI units; nb_k is monotone; the descriptor marks the kind of grid by the sign of h."""
+    t = 2000.0 + np.arange(0.0, 2 * 27.4, 1.0 / 48.0)           # 2 continuous sectors, 30-min cadence
+    rho = 1.7
+    g0 = orc.grid(cfg, t, rho)
+    f0, nb0 = orc.freqs(cfg, g0)
+    cu = orc.default_config(uniform_freq=1)
+    gu = orc.grid(cu, t, rho)
+    fu, nbu = orc.freqs(cu, gu)
+    assert gu["status"] == 0 and gu["h"] < 0 < g0["h"] and gu["u0"] == 1.0 / g0["p_max"]
+    for k in ("t_ref", "baseline", "p_min", "p_max", "c_q", "nb_max"):
+        assert gu[k] == g0[k]
+    # arithmetic progression over the same range
+    assert fu[0] == 1.0 / g0["p_max"] and fu[0] == pytest.approx(f0[0], rel=1e-15)
+    assert fu[-1] <= (1.0 / g0["p_min"]) * (1 + 1e-12)
+    assert fu[-1] + (-gu["h"]) > 1.0 / g0["p_min"]
+    assert np.allclose(np.diff(fu), -gu["h"], rtol=1e-9) and np.all(np.diff(fu) > 0)
+    assert fu.size == gu["n_freq"] == int(math.floor((1.0 / g0["p_min"] - fu[0]) / -gu["h"])) + 1
+    # its step = the finest step of the GPU grid (at the low-frequency end): 3 u0^2 h to first order
+    assert -gu["h"] == pytest.approx(f0[1] - f0[0], rel=3.0 * g0["h"] / g0["u0"])
+    assert -gu["h"] < np.diff(f0).min() * (1 + 1e-12)
+    assert fu.size > 3 * f0.size                                 # uniform steps need many more points
+    # Keplerian nb at f_k, from Kepler III in SI units (exact ceil except within 1e-9 of an integer)
+    q_lo = 0.5 / (math.pi * a_over_r(1.0 / fu, rho))
+    x = 3.0 / q_lo
+    safe = np.abs(x - np.round(x)) > 1e-6
+    assert safe.mean() > 0.999 and np.array_equal(nbu[safe], np.ceil(x[safe]).astype(np.int32))
+    assert nbu[0] == gu["nb_max"] and nbu[-1] == 38 and np.all(np.diff(nbu) <= 0)
+    # capped: exactly M points, both ends kept
+    for M in (80000, 1000, 2):
+        cm = orc.default_config(uniform_freq=1, max_freq=M)
+        gm = orc.grid(cm, t, rho)
+        fm, nbm = orc.freqs(cm, gm)
+        if gu["n_freq"] <= M:
+            assert gm.tobytes() == gu.tobytes()
+            continue
+        assert fm.size == gm["n_freq"] == M and fm[0] == fu[0]
+        assert fm[-1] == pytest.approx(1.0 / g0["p_min"], rel=1e-13)
+        assert np.allclose(np.diff(fm), (1.0 / g0["p_min"] - fm[0]) / (M - 1), rtol=1e-9)
+        assert np.all(np.diff(nbm) <= 0) and nbm[0] == gu["nb_max"] and nbm[-1] == 38
+    # the comparison workload as SURVEY.md 8(f) words it: uniform, <= 80,000 frequencies, P <= 56 d; context of
+    # PAPER.md:59 ("up to ~10 times more frequencies" on the GPU grid) on the longest baseline
+    comp = orc.default_config(uniform_freq=1, max_period_days=56.0, max_freq=80000)
+    t40 = 2000.0 + np.arange(0.0, 40 * 27.4, 1.0 / 48.0)
+    for rho_s, lo, hi in ((10.0, 5.0, 15.0), (1.0, 2.0, 4.0)):
+        gc = orc.grid(comp, t40, rho_s)
+        assert gc["n_freq"] == 80000 and gc["p_max"] == 56.0 and gc["h"] < 0
+        assert lo < orc.grid(cfg, t40, rho_s)["n_freq"] / 80000 < hi
+    # a step below 1e-9 f_max is refused
+    tiny = orc.grid(orc.default_config(uniform_freq=1, samples_per_peak=1e9), t, rho)
+    assert tiny["status"] == 3 and tiny["n_freq"] == 0
+    # degenerate stars keep their status
+    assert orc.grid(cu, t[:1], rho)["status"] == 1
+
+
+def test_search_on_the_uniform_comparison_grid_recovers_an_injection(orc):
+    """End to end on the frequency-uniform grid: the spectrum at index k is the spectrum of (f_k, nb_k) of that grid
+    (brute force through sr_one), and the injected period of BASELINE.json configs[0] is found to within one step."""
+    comp = orc.default_config(uniform_freq=1, max_freq=3000)
+    b = synth.make_batch(1, n_stars=1)
+    t, y, dy = b.star(0)
+    out = orc.batch(comp, b.row_ptr, b.t, b.y, b.dy, b.rho, K=1, want_snr=True)
+    g = out["grid"][0:1]
+    f, nb = orc.freqs(comp, g)
+    assert f.size == 3000 and g["h"][0] < 0
+    tau, w, wy = orc.prep(t, y, dy, float(g["t_ref"][0]))[:3]
+    M = orc.widths(comp)
+    for k in (0, 1, 1499, 2999):
+        sr, m, j = orc.sr_one(tau, w, wy, float(f[k]), int(nb[k]), M)[:3]
+        assert out["sr"][k] == sr and out["m"][k] == m and out["j"][k] == j
+    pk = out["peaks"][0][0]
+    truth = b.truth[0]
+    assert pk["freq"] == f[pk["k"]]
+    n = round(pk["period"] / truth["period"]) if pk["period"] > truth["period"] else 1
+    assert abs(1.0 / pk["period"] - 1.0 / (n * truth["period"])) < 2.0 * -g["h"][0]
+
+
 def test_grid_invariances(orc, cfg):
     t, *_ = synth.make_star(3, 11)
     g = orc.grid(cfg, t, 1.7)

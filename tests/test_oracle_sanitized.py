@@ -66,6 +66,8 @@ for s in range(bb.n_stars):
 # the comparison grid's caps
 cc = O.default_config(max_period_days=12.0, max_freq=500)
 O.batch(cc, b.row_ptr, b.t, b.y, b.dy, b.rho, K=3, want_snr=True, threads=1)
+cu = O.default_config(uniform_freq=1, max_period_days=12.0, max_freq=500)   # O1.10c: equal steps in frequency
+O.batch(cu, b.row_ptr, b.t, b.y, b.dy, b.rho, K=3, want_snr=True, threads=1)
 print("sanitized oracle ok")
 '''
 
