@@ -780,13 +780,21 @@ def main():
     ap.add_argument("--comparison-grid", action="store_true",
                     help="search the comparison grid of DESIGN.md O1.10 (PAPER.md:13: periods up to 56 d, at most "
                          "80,000 frequencies per star) instead of the paper's GPU grid")
+    ap.add_argument("--comparison-grid-uniform", action="store_true",
+                    help="the same caps on a grid with equal steps in FREQUENCY (DESIGN.md O1.10c: the comparison "
+                         "workload as SURVEY.md 8(f) words it)")
     ap.add_argument("--ref-budget", type=float, default=4.0, help="--impl reference: seconds of oracle work per step")
     args = ap.parse_args()
     if args.stars is None:
         from paper_2302_01293_b200 import synth
         args.stars = DEFAULT_STARS if args.config == 5 else min(synth.N_STARS[args.config], 1000)
-    if args.comparison_grid:
+    if args.comparison_grid or args.comparison_grid_uniform:
         GRID_KW.update(max_period_days=56.0, max_freq=80000)
+    if args.comparison_grid_uniform:
+        global GRID_NOTE
+        GRID_KW.update(uniform_freq=1)
+        GRID_NOTE = ("comparison grid O1.10c (PAPER.md:13; SURVEY.md 8(f) f4): equal steps in frequency, P <= 56 d, "
+                     "<= 80,000 frequencies per star")
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.chunk == 0:
         respawn_under_torchrun(args)

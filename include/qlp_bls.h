@@ -71,12 +71,18 @@ typedef struct {
   uint32_t flags;           /* bit0: validate inputs on the device (t finite and strictly
                                increasing in qlp_bls_grid; y, dy finite and dy > 0 in
                                qlp_bls_spectrum, which then synchronises once); a violation makes
-                               the call return QLP_BLS_EVALIDATION.  Other bits reserved (0)      */
+                               the call return QLP_BLS_EVALIDATION.
+                               bit1: the comparison grid has equal steps in FREQUENCY (see below;
+                               read by qlp_bls_grid only).  Other bits reserved (0)                */
   uint32_t reserved_;       /* 0                                                                 */
   /* Comparison grid (O1.10; the earlier CPU search used "an under-sampled
    * frequency grid on the order of 80,000 frequencies or less" and "periods up to only ~56 days").
    * Both 0 (default) = the paper's GPU grid.  Only qlp_bls_grid reads them.  qlp_bls_create returns
-   * QLP_BLS_EINVAL for max_period_days < 0 (or NaN), max_freq < 0 or max_freq == 1.              */
+   * QLP_BLS_EINVAL for max_period_days < 0 (or NaN), max_freq < 0 or max_freq == 1.
+   * flags bit1 (O1.10c; "uniform <= 80,000-frequency grid, P <= 56 d"): f_k = f_min + k df
+   * over the same range [1 / p_max, 1 / p_min] instead of equal steps in f^(1/3); df = the step of the f^(1/3) law
+   * at f_min (its finest), or (f_max - f_min) / (max_freq - 1) when that takes more than max_freq points.  nb_k
+   * keeps the Keplerian law at f_k.  A star whose step would be below 1e-9 f_max gets status 3.                */
   double max_period_days;   /* > 0: P_max = min(P_max, max_period_days)                          */
   int64_t max_freq;         /* >= 2: a star whose grid has more frequencies gets exactly max_freq
                                of them over the same range, step (u1 - u0) / (max_freq - 1)      */
@@ -84,18 +90,22 @@ typedef struct {
 
 /* Per-star grid descriptor, written by qlp_bls_grid() (device memory, one per star).
  * Frequency k of the star is f_k = u^3 with u = u0 + k*h (FP64, in that order), and its number
- * of fine phase bins is nb_k = ceil(noverlap / (qmin_fac * c_q * u^2)).  DESIGN.md O1. */
+ * of fine phase bins is nb_k = ceil(noverlap / (qmin_fac * c_q * u^2)).  DESIGN.md O1.
+ * On the frequency-uniform comparison grid (flags bit1) h is NEGATIVE and marks the kind of grid:
+ * f_k = u0 + k*(-h) with u0 = 1 / p_max, and nb_k by the same formula with u = cbrt_det(f_k). */
 typedef struct {
   double t_ref;     /* first timestamp: phase zero point (reading A4)                            */
   double baseline;  /* T = t_last - t_first, days                                                */
   double p_min;     /* period at which a = a_over_rstar_min * R*   PAPER.md:23                    */
   double p_max;     /* longest continuous stretch, or half of it                    */
   double c_q;       /* q_circ(f) = c_q * f^(2/3)                    */
-  double u0;        /* cbrt_det(1 / p_max)                                                       */
-  double h;         /* grid step in u = f^(1/3)                    PAPER.md:35 (samples_per_peak) */
+  double u0;        /* cbrt_det(1 / p_max)   (flags bit1: 1 / p_max)                             */
+  double h;         /* grid step in u = f^(1/3)                    PAPER.md:35 (samples_per_peak)
+                       (flags bit1: minus the step in frequency)                                 */
   int64_t n_freq;   /* number of trial frequencies                                               */
   int32_t nb_max;   /* phase bins at k = 0 (the largest)                                         */
-  int32_t status;   /* 0 ok; 1 fewer than 2 points; 2 baseline <= 0; 3 f_max <= f_min;
+  int32_t status;   /* 0 ok; 1 fewer than 2 points; 2 baseline <= 0; 3 f_max <= f_min (or, flags
+                       bit1, a frequency step below 1e-9 f_max);
                        4 nb_max > QLP_BLS_MAX_NB (star skipped, n_freq = 0);
                        5 more than QLP_BLS_MAX_POINTS points (star skipped, n_freq = 0);
                        7 timestamps not finite and strictly increasing (star skipped, n_freq = 0:

@@ -99,8 +99,11 @@ def load_library(check: bool = False):
 def default_config(**kw) -> Config:
     cfg = Config()
     load_library().qlp_bls_default_config(C.byref(cfg))
+    uniform = kw.pop("uniform_freq", None)
     for k, v in kw.items():
         setattr(cfg, k, v)
+    if uniform is not None:                # flags bit 1: comparison grid with equal steps in frequency (O1.10c)
+        cfg.flags = (cfg.flags | 2) if uniform else (cfg.flags & ~2)
     return cfg
 
 
@@ -219,11 +222,12 @@ class QlpBls:
         """qlp_bls_spectrum -> (sr float32[total_freq], best uint32-as-int32[total_freq])."""
         torch = self.torch
         S = int(row_ptr.numel()) - 1
-        sr = torch.empty(max(total_freq, 1), dtype=torch.float32, device=self.device)[:total_freq]
-        best = torch.empty(max(total_freq, 1), dtype=torch.int32, device=self.device)[:total_freq]
+        # at least one element each, so that a batch without any frequency still hands over valid pointers
+        sr = torch.empty(max(total_freq, 1), dtype=torch.float32, device=self.device)
+        best = torch.empty(max(total_freq, 1), dtype=torch.int32, device=self.device)
         _check(self.lib.qlp_bls_spectrum(self._h, S, _ptr(row_ptr), _ptr(t), _ptr(y), _ptr(dy), _ptr(grid),
                                          _ptr(freq_ptr), _ptr(sr), _ptr(best), self._stream()), "qlp_bls_spectrum")
-        return sr, best
+        return sr[:total_freq], best[:total_freq]
 
     def spectrum_into(self, row_ptr, t, y, dy, grid, freq_ptr, sr, best):
         S = int(row_ptr.numel()) - 1

@@ -153,6 +153,7 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
   p.qmax_fac = cfg->qmax_fac; p.a_over_rstar_min = cfg->a_over_rstar_min; p.sector_days = cfg->sector_days;
   p.noverlap = cfg->noverlap; p.top_k = cfg->top_k;
   p.max_period_days = cfg->max_period_days; p.max_freq = cfg->max_freq;
+  p.uniform_freq = (cfg->flags & 2u) ? 1 : 0;
   p.wmask = 0; p.max_width = 0; p.min_width = ctx->widths[0];
   for (int i = 0; i < ctx->n_widths; ++i) {
     int m = ctx->widths[i];
@@ -445,7 +446,9 @@ extern "C" int qlp_bls_spectrum(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t
     const int per_sm = class_ctas_per_sm(c);
     const unsigned nblk = (unsigned)(ctx->n_sm * per_sm);
     const int64_t* off_c = off + (int64_t)c * (n_stars + 1);
-    const bool generic = ctx->prm.wmask != kPaperMask;  // the paper's ladder {3..11} is compiled in
+    // the paper's ladder {3..11} is compiled in; other ladders and the frequency-uniform comparison grid (O1.10c)
+    // run the kernels with the run-time ladder, the only ones that know that grid
+    const bool generic = ctx->prm.wmask != kPaperMask || ctx->prm.uniform_freq != 0;
 #define QLP_LAUNCH(MW_, CT_, WM_)                                                                                          \
   foldscan_kernel<MW_, CT_, WM_><<<nblk, kThreads, smem, st>>>(ctx->prm, c, n_stars, row_ptr, (const Point*)ctx->pts.p,    \
                                                          (const StarPrep*)ctx->prep.p, grid, freq_ptr, off_c, kb,    \

@@ -51,6 +51,7 @@ struct Params {
   uint32_t wmask;     // bit m set <=> width m is on the ladder (O1.9)
   int32_t max_width;  // largest width
   int32_t min_width;  // smallest width (the all-zero answer, O4)
+  int32_t uniform_freq;  // O1.10c: comparison grid with equal steps in frequency (flags bit 1); read by grid_kernel only
 };
 
 
@@ -93,13 +94,27 @@ __device__ inline double cbrt_det(double x) {
 }
 
 // O1.8: frequency k of a star and its number of fine bins.  Q = qmin_fac * c_q.
-__device__ __forceinline__ void freq_of_k(double u0, double h, double Q, double noverlap, int64_t k,
-                                          double& f, int32_t& nb) {
+// freq_of_k_cube: the f^(1/3) law alone (h > 0), without the test for the other kind of grid -- what the fold kernels
+// compiled for the paper's ladder call, so that their code is the same whether or not the library knows the
+// comparison grid.  freq_of_k (below): either kind, by the sign of h; everything else calls that one.
+__device__ __forceinline__ void freq_of_k_cube(double u0, double h, double Q, double noverlap, int64_t k,
+                                               double& f, int32_t& nb) {
   double u = dadd(u0, dmul((double)k, h));
   double u2 = dmul(u, u);
   f = dmul(u2, u);
   double qlo = dmul(Q, u2);
   nb = (int32_t)ceil(ddiv(noverlap, qlo));
+}
+
+__device__ __forceinline__ void freq_of_k(double u0, double h, double Q, double noverlap, int64_t k,
+                                          double& f, int32_t& nb) {
+  if (h < 0.0) {  // O1.10c: the descriptor of a frequency-uniform grid holds u0 = f_min and h = -df
+    f = dadd(u0, dmul((double)k, -h));
+    const double uk = cbrt_det(f);
+    nb = (int32_t)ceil(ddiv(noverlap, dmul(Q, dmul(uk, uk))));
+    return;
+  }
+  freq_of_k_cube(u0, h, Q, noverlap, k, f, nb);
 }
 
 // O3: bin of one point.  p = fl64(f * tau) is the only rounded operation; the bin is

@@ -147,6 +147,17 @@ struct TileInfo {
 // costs two shared-memory wavefronts, the two atomics of an evaluation one each, and the
 // shared-memory pipe (one wavefront per clock per SM) is what binds.
 // With CTOT < 32 the spare lanes take 32/CTOT consecutive points.
+// (f_k, nb_k) inside the fold kernel.  Only the kernels with the run-time ladder (WM == 0) know the
+// frequency-uniform comparison grid (O1.10c; the host sends such a context to them): the kernels compiled for the
+// paper's ladder keep the branch-free f^(1/3) law, so the comparison grid costs the headline path nothing -- with
+// the test inlined into them the 64-column class lost 4.6 % to a different register allocation of its inner loop.
+template <bool ANY_GRID>
+__device__ __forceinline__ void tile_freq_of_k(double u0, double h, double Q, double noverlap, int64_t k, double& f,
+                                               int32_t& nb) {
+  if (ANY_GRID) freq_of_k(u0, h, Q, noverlap, k, f, nb);
+  else freq_of_k_cube(u0, h, Q, noverlap, k, f, nb);
+}
+
 template <int MW, int CTOT, uint32_t WM>
 __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kernel(
     Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
@@ -231,7 +242,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         x.u0 = g.u0; x.h = g.h; x.Q = dmul(prm.qmin_fac, g.c_q);
         x.inv_w = sp.inv_w; x.inv_s = sp.inv_s;
         double f; int32_t nb;
-        freq_of_k(x.u0, x.h, x.Q, dno, x.k0, f, nb);
+        tile_freq_of_k<WM == 0u>(x.u0, x.h, x.Q, dno, x.k0, f, nb);
         x.nb_tile = nb;
         // start streaming the first two chunks of the star's points
         const Point* src = pts + x.pt_begin;
@@ -274,7 +285,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
         lane_off[r] = (uint32_t)((PAIRED || QUAD) ? col : col0) * 4u;
         f[r] = 0.0;
         int32_t nbk = 1;
-        if (col < ti.ncols) freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
+        if (col < ti.ncols) tile_freq_of_k<WM == 0u>(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
         dnb[r] = (double)nbk;
         neg_nb_row[r] = 0u - (uint32_t)nbk * (uint32_t)(STRIDE * 4);
       }
@@ -361,7 +372,7 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
     int32_t nbk = 1;
     if (scol_on) {
       double fk;
-      freq_of_k(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, fk, nbk);
+      tile_freq_of_k<WM == 0u>(ti.u0, ti.h, ti.Q, dno, ti.k0 + scol, fk, nbk);
       const int per = (nbk + TPC - 1) / TPC;
       const int ja = seg * per;
       const int jb = min(nbk, ja + per);

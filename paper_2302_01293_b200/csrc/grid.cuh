@@ -117,7 +117,20 @@ __global__ void __launch_bounds__(256) grid_kernel(Params prm, int64_t n_stars, 
           q.u0 = u0; q.h = h;
           double qlo = dmul(Q, dmul(u0, u0));
           q.nb_max = (int32_t)ceil(ddiv((double)prm.noverlap, qlo));
-          if (bad_t) { q.status = 7; q.n_freq = 0; }
+          // O1.10c: equal steps in frequency over the same range; df = the f^(1/3) law's step at f_min (A u0^2),
+          // or (f_max - f_min) / (max_freq - 1) when that takes more than max_freq points; u0 <- f_min, h <- -df
+          if (prm.uniform_freq) {
+            double df = dmul(A, dmul(u0, u0));
+            q.n_freq = (int64_t)floor(ddiv(dsub(f_max, f_min), df)) + 1;
+            if (prm.max_freq >= 2 && q.n_freq > prm.max_freq) {
+              df = ddiv(dsub(f_max, f_min), (double)(prm.max_freq - 1));
+              q.n_freq = prm.max_freq;
+            }
+            if (!(df > dmul(1e-9, f_max))) { q.status = 3; q.n_freq = 0; q.nb_max = 0; q.u0 = 0.0; q.h = 0.0; }
+            else { q.u0 = f_min; q.h = -df; }
+          }
+          if (q.status == 3) { }
+          else if (bad_t) { q.status = 7; q.n_freq = 0; }
           else if (q.nb_max > QLP_BLS_MAX_NB || q.nb_max <= 0) { q.status = 4; q.n_freq = 0; }
           else if (n >= (int64_t)QLP_BLS_MAX_POINTS) { q.status = 5; q.n_freq = 0; }  // fixed-point weights
         }

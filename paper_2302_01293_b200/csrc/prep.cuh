@@ -110,7 +110,11 @@ __global__ void __launch_bounds__(256) prep_kernel(Params prm, int64_t n_stars, 
     double cnt = (double)n;
     if (g.status == 0 && g.n_freq > 0) {
       const double Q = prm.qmin_fac * g.c_q;
-      const double u_lo = g.u0, u_hi = g.u0 + (double)g.n_freq * g.h;
+      double u_lo = g.u0, u_hi = g.u0 + (double)g.n_freq * g.h;
+      if (g.h < 0.0) {  // frequency-uniform grid (O1.10c): u0 = f_min, h = -df
+        u_lo = cbrt_det(g.u0);
+        u_hi = cbrt_det(g.u0 + (double)g.n_freq * (-g.h));
+      }
       const double no = (double)prm.noverlap;
       // sum over cycles of D/d: D = Q/(no u) days per bin and cycle, C = f T + 2 cycles, evaluated at the grid
       // ends (u_hi for the f T part, u_lo for the + 2 part); cycles = C at the highest frequency

@@ -348,7 +348,10 @@ def test_comparison_grid_long_baseline(gpu, orc):
                                 dict(noverlap=4, dlogq=0.2),                       # ladder {4,5,6,7,8,10,12,14}: gaps, width 14
                                 dict(noverlap=2, qmax_fac=3.0),                    # ladder {2..11}
                                 dict(noverlap=5, dlogq=0.05, qmax_fac=1.5),        # ladder {5..15}
-                                dict(max_period_days=5.0, max_freq=1500)])         # O1.10 caps, both biting on config 2
+                                dict(max_period_days=5.0, max_freq=1500),          # O1.10 caps, both biting on config 2
+                                dict(uniform_freq=1),                              # O1.10c: equal steps in frequency, uncapped
+                                dict(uniform_freq=1, max_period_days=5.0, max_freq=1500),
+                                dict(uniform_freq=1, samples_per_peak=1e9)])       # step below 1e-9 f_max: status 3
 def test_other_search_parameters(gpu, orc, kw):
     """Non-default qlp_bls_config: grid bit-exact and SR parity with the oracle under the same parameters.
     Ladders other than the paper's {3..11} run the generic (run-time mask, 16-wide window) kernel."""
@@ -365,8 +368,12 @@ def test_other_search_parameters(gpu, orc, kw):
         sr, best = ctx.spectrum(dev[0], dev[1], dev[2], dev[3], grid, freq_ptr, tf)
         sr, best, fp = sr.cpu().numpy(), best.cpu().numpy(), freq_ptr.cpu().numpy()
         ob = orc.batch(ocfg, b.row_ptr, b.t, b.y, b.dy, b.rho, K=0, want_snr=False)
+        if kw.get("samples_per_peak", 0) > 1e6:                # the refused grid: no frequencies, nothing searched
+            assert np.all(go["status"] == 3) and int(tf) == 0
         for s in range(b.n_stars):
             a, e = int(fp[s]), int(fp[s + 1])
+            if e == a:
+                continue
             rel, same, m_g, j_g = _compare_sr(sr[a:e], best[a:e], ob["sr"][a:e], ob["m"][a:e], ob["j"][a:e], f"{kw}[{s}]")
             assert same > 0.98
             assert set(np.unique(m_g)) <= set(orc.widths(ocfg).tolist())

@@ -317,6 +317,43 @@ def test_snr_at_production_grid_sizes(gpu, ctx, orc, cfg):
           f"(Sturges N = {orc.sturges(nf_best)}) worst {w5:.2e} of max|S/N|")
 
 
+def test_uniform_comparison_grid_long_baseline(gpu, orc):
+    """O1.10c, the comparison workload as SURVEY.md 8(f) f4 words it (equal steps in frequency, <= 80,000
+    frequencies, P <= 56 d) on 13-sector, 200-s stars (config 4): descriptors (h < 0) and sampled
+    (f_k, nb_k) bit-exact; SR and (m, j) on 400 frequencies per star spread over every tile class the grid reaches;
+    S/N and the peak table against the oracle fed the GPU's SR."""
+    from paper_2302_01293_b200 import synth
+    kw = dict(uniform_freq=1, max_period_days=56.0, max_freq=80000)
+    ocfg = orc.default_config(**kw)
+    b = synth.make_batch(4, n_stars=2)
+    ctx = gpu.QlpBls(**kw)
+    try:
+        res = _search(gpu, ctx, b, want_snr=True)
+        go = _oracle_grids(orc, ocfg, b)
+        assert res["grid"].tobytes() == go.tobytes()
+        assert np.all(go["h"] < 0) and np.all(go["u0"] == 1.0 / 56.0) and np.all(go["n_freq"] == 80000)
+        rng = np.random.default_rng(5)
+        for s in range(b.n_stars):
+            for k0 in (0, 40000, 80000 - 64):
+                f, nb = ctx.debug_freqs(res["grid_dev"], s, k0, k0 + 64)
+                fo, nbo = orc.freqs(ocfg, go[s], k0, k0 + 64)
+                assert np.array_equal(f.cpu().numpy(), fo) and np.array_equal(nb.cpu().numpy(), nbo)
+            # equal steps in f put most points at small nb: sample the low-frequency end densely as well
+            ks = np.unique(np.concatenate([[0, 1, 2, 79999], rng.integers(0, 80000, 200),
+                                           (rng.random(200) ** 3 * 80000).astype(np.int64)]))
+            _, nbs = orc.freqs(ocfg, go[s])
+            classes = {_class_of(int(nbs[k])) for k in ks}
+            assert classes >= set(range(0, _class_of(int(go[s]["nb_max"])) + 1))
+            a, e = int(res["fp"][s]), int(res["fp"][s + 1])
+            worst, same = _check_sampled(orc, ocfg, b, s, go[s], res, ks, peak=float(res["sr"][a:e].max()))
+            print(f"uniform comparison grid, star {s}: nb {int(go[s]['nb_max'])}..38, classes {sorted(classes)}, "
+                  f"worst |dSR|/peak = {worst:.2e}, (m,j) identical on {same:.4f}")
+            assert same > 0.97
+        _check_snr_given_gpu_sr(gpu, ctx, orc, ocfg, b, res, go, range(b.n_stars))
+    finally:
+        ctx.close()
+
+
 # ---------------------------------------------------------------------------------------------- (e)
 def test_s_scale_with_near_coincident_timestamps(gpu, ctx, orc, cfg):
     """40 sectors at 200 s (456,000 points) with a few timestamp pairs 1e-6 d apart (overlapping sectors or
