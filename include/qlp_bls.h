@@ -73,7 +73,8 @@ typedef struct {
                                qlp_bls_spectrum, which then synchronises once); a violation makes
                                the call return QLP_BLS_EVALIDATION.
                                bit1: the comparison grid has equal steps in FREQUENCY (see below;
-                               read by qlp_bls_grid only).  Other bits reserved (0)                */
+                               read by qlp_bls_grid only).  Other bits reserved: qlp_bls_create
+                               returns QLP_BLS_EINVAL unless they (and reserved_) are 0            */
   uint32_t reserved_;       /* 0                                                                 */
   /* Comparison grid (O1.10; the earlier CPU search used "an under-sampled
    * frequency grid on the order of 80,000 frequencies or less" and "periods up to only ~56 days").

@@ -141,7 +141,8 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
   if (!(cfg->samples_per_peak > 0.0) || !(cfg->dlogq > 0.0) || cfg->noverlap < 1 || cfg->noverlap > kMaxWidth ||
       !(cfg->qmin_fac > 0.0) || !(cfg->qmax_fac >= cfg->qmin_fac) || !(cfg->a_over_rstar_min > 0.0) ||
       !(cfg->sector_days > 0.0) || cfg->top_k < 1 || cfg->top_k > kMaxTopK ||
-      !(cfg->max_period_days >= 0.0) || cfg->max_freq < 0 || cfg->max_freq == 1)
+      !(cfg->max_period_days >= 0.0) || cfg->max_freq < 0 || cfg->max_freq == 1 ||
+      (cfg->flags & ~3u) != 0u || cfg->reserved_ != 0u)   // reserved bits must be 0, so that they can get a meaning
     return QLP_BLS_EINVAL;
   qlp_bls_ctx* ctx = new (std::nothrow) qlp_bls_ctx();
   if (!ctx) return QLP_BLS_ENOMEM;

@@ -54,7 +54,7 @@ def test_strerror_and_bad_args(lib):
     cfg = bls.default_config(top_k=99)
     h = C.c_void_p()
     assert lib.qlp_bls_create(C.byref(cfg), C.byref(h)) == -1
-    for bad in (dict(max_freq=1), dict(max_freq=-5), dict(max_period_days=-1.0)):
+    for bad in (dict(max_freq=1), dict(max_freq=-5), dict(max_period_days=-1.0), dict(flags=4), dict(reserved_=1)):
         assert lib.qlp_bls_create(C.byref(bls.default_config(**bad)), C.byref(h)) == -1
     cfg = bls.default_config(a_over_rstar_min=0.5)  # boxes would be wider than the histogram
     assert lib.qlp_bls_create(C.byref(cfg), C.byref(h)) == -1
