@@ -158,8 +158,18 @@ __device__ __forceinline__ void tile_freq_of_k(double u0, double h, double Q, do
   else freq_of_k_cube(u0, h, Q, noverlap, k, f, nb);
 }
 
+// Register budget of the fold kernels, through __launch_bounds__(T, B): ptxas keeps a kernel within 65536 / (T * B)
+// registers per thread (T >= kThreads: the launches use kThreads).  128 columns: 64 registers, the budget of two
+// CTAs per SM (class 0).  The other caps are tuning, measured per class on config 5: the
+// 32-column (paired) loop is 8 % faster at 56 registers than with the 75 ptxas takes when left alone (0.415 -> 0.449
+// of the peak; 64: 0.422, 48: 0.407, 40 with spills: 0.396), the 64-column loop 2 % faster at 72 (70 used; 78
+// uncapped: 0.506 -> 0.515; 64: 0.498).  Giving class 1 a build of its own with more than 64 registers made it
+// slower (72: 0.572, 94: 0.549, 118 with 8 points in flight: 0.534, against 0.590), and so did every cap tried on
+// the 16-column class (71: 0.297, 64: 0.289, 56: 0.286, against 0.307 at 79).
+template <int CTOT> constexpr int fold_lb_threads() { return CTOT == 64 ? 832 : (CTOT == 32 ? 576 : kThreads); }
+template <int CTOT> constexpr int fold_lb_blocks() { return (CTOT == 128 || CTOT == 32) ? 2 : 1; }
 template <int MW, int CTOT, uint32_t WM>
-__global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kernel(
+__global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>()) foldscan_kernel(
     Params prm, int cls, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const int64_t* __restrict__ tile_off, const int64_t* __restrict__ kb,
@@ -191,7 +201,10 @@ __global__ void __launch_bounds__(kThreads, (CTOT == 128 ? 2 : 1)) foldscan_kern
   constexpr int HPW = 32 / CW;                  // points per warp iteration
   constexpr int STEP = kWarps * HPW;            // points consumed per iteration by the CTA
   constexpr int ITERS = kChunk / STEP;
-  constexpr int U = ITERS < 4 ? ITERS : 4;      // points in flight per lane
+  // points in flight per lane: 4 (2 and 8 measured slower in every class down to 16 columns); the 8-column class
+  // takes its whole chunk share of 8 (0.195 -> 0.214 of the peak)
+  constexpr int UW = (CTOT == 8) ? 8 : 4;
+  constexpr int U = ITERS < UW ? ITERS : UW;
   static_assert(ITERS >= 1 && ITERS % U == 0, "chunk must be a multiple of the CTA's point step");
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int col0 = lane % CW;                   // first column of this lane in the fold phase
