@@ -325,29 +325,14 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
           __syncthreads();
         }
         const int4* p4 = reinterpret_cast<const int4*>(buf) + warp * HPW + hsub;
-#ifdef QLP_SWPIPE
-        constexpr bool SWP = (CTOT >= QLP_SWPIPE) && (U == 4);
-#else
-        constexpr bool SWP = false;
-#endif
-        int4 v[U];
-        if (SWP) {
-#pragma unroll
-          for (int u = 0; u < U; ++u) v[u] = p4[u * STEP];
-        }
 #pragma unroll 1
         for (int it = 0; it < ITERS; it += U) {
-          if (!SWP) {
+          int4 v[U];
 #pragma unroll
-            for (int u = 0; u < U; ++u) v[u] = p4[(it + u) * STEP];
-          }
+          for (int u = 0; u < U; ++u) v[u] = p4[(it + u) * STEP];
 #pragma unroll
           for (int u = 0; u < U; ++u) {
-            const int4 vu = v[u];
-            // software pipeline: the slot just consumed is refilled with the point of the next iteration (the last
-            // iteration reads past the chunk into shared memory that is never used)
-            if (SWP) v[u] = p4[(it + U + u) * STEP];
-            const double tau = __hiloint2double(vu.y, vu.x);
+            const double tau = __hiloint2double(v[u].y, v[u].x);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
               // byte offset of the bin's row: (I - nb g) * row bytes, as I * row + g * (-nb row) (+ lane)
@@ -361,14 +346,14 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
                                                        (uint32_t)CTOT))
                 continue;
               if (HPW == 1 || PAIRED) {
-                atomicAdd(cell, (uint32_t)vu.z);
-                atomicAdd(cell + CTOT, (uint32_t)vu.w);
+                atomicAdd(cell, (uint32_t)v[u].z);
+                atomicAdd(cell + CTOT, (uint32_t)v[u].w);
               } else {
                 // Narrow classes: the lanes that share a column fold different points, and with a row of
                 // 2*CTOT <= 32 words they would meet on one bank in both atomics.  Odd point-lanes therefore
                 // add S first and W second: in each instruction the two parities use different banks.
-                atomicAdd(cell + first_off, swap_ws ? (uint32_t)vu.w : (uint32_t)vu.z);
-                atomicAdd(cell + (CTOT - first_off), swap_ws ? (uint32_t)vu.z : (uint32_t)vu.w);
+                atomicAdd(cell + first_off, swap_ws ? (uint32_t)v[u].w : (uint32_t)v[u].z);
+                atomicAdd(cell + (CTOT - first_off), swap_ws ? (uint32_t)v[u].z : (uint32_t)v[u].w);
               }
             }
           }
