@@ -296,6 +296,8 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
       for (int r = 0; r < R; ++r) {
         const int col = col0 + CW * ((PAIRED || QUAD) ? (r ^ (hsub & 1)) : r);
         lane_off[r] = (uint32_t)((PAIRED || QUAD) ? col : col0) * 4u;
+        // lanes that add S first (see below) start CTOT words further: folded into the lane's offset here
+        if (HPW > 1 && !PAIRED) lane_off[r] += (uint32_t)(((QUAD ? (hsub & 2) != 0 : (hsub & 1) != 0) ? CTOT : 0) * 4);
         f[r] = 0.0;
         int32_t nbk = 1;
         if (col < ti.ncols) tile_freq_of_k<WM == 0u>(ti.u0, ti.h, ti.Q, dno, ti.k0 + col, f[r], nbk);
@@ -306,7 +308,7 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
       const Point* src = pts + ti.pt_begin;
       const int64_t n_chunks = (n + kChunk - 1) / kChunk;
       const bool swap_ws = (HPW > 1) && !PAIRED && (QUAD ? (hsub & 2) != 0 : (hsub & 1) != 0);
-      const int first_off = swap_ws ? CTOT : 0;
+      const uint32_t sel_first = swap_ws ? 0x7654u : 0x3210u, sel_second = swap_ws ? 0x3210u : 0x7654u;  // W,S or S,W
       unsigned char* hbytes = reinterpret_cast<unsigned char*>(hist);
       __syncthreads();  // histograms zeroed
       clk1s = phase ? clock64() : 0;
@@ -325,7 +327,9 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
           __syncthreads();
         }
         const int4* p4 = reinterpret_cast<const int4*>(buf) + warp * HPW + hsub;
-#pragma unroll 1
+        // the 64-column kernel gains 1.3 % from two iterations per loop trip (the 128-column ones lose 3-6 %)
+        constexpr int UNR_IT = (CTOT == 64) ? 2 : 1;
+#pragma unroll UNR_IT
         for (int it = 0; it < ITERS; it += U) {
           int4 v[U];
 #pragma unroll
@@ -347,9 +351,10 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
               const uint32_t off = g * neg_nb_row[r] + (I * (uint32_t)(STRIDE * 4) + lane_off[r]);
               uint32_t* cell = reinterpret_cast<uint32_t*>(hbytes + off) + ((PAIRED || QUAD) ? 0 : CW * r);
               // check build: the cell lies inside this tile's histogram (bin < nb of the column <= nb_tile)
+              // (the narrow classes' lanes that add S first start in the S half of the row: up to 2 CTOT words)
               if (!QLP_IN_BOUNDS(kChkFoldCell, off / (uint32_t)(STRIDE * 4) < (uint32_t)nb_tile &&
                                                    (off % (uint32_t)(STRIDE * 4)) / 4u + (uint32_t)((PAIRED || QUAD) ? 0 : CW * r) <
-                                                       (uint32_t)CTOT))
+                                                       (uint32_t)((HPW > 1 && !PAIRED) ? STRIDE : CTOT)))
                 continue;
               if (HPW == 1 || PAIRED) {
                 atomicAdd(cell, (uint32_t)v[u].z);
@@ -358,8 +363,13 @@ __global__ void __launch_bounds__(fold_lb_threads<CTOT>(), fold_lb_blocks<CTOT>(
                 // Narrow classes: the lanes that share a column fold different points, and with a row of
                 // 2*CTOT <= 32 words they would meet on one bank in both atomics.  Odd point-lanes therefore
                 // add S first and W second: in each instruction the two parities use different banks.
-                atomicAdd(cell + first_off, swap_ws ? (uint32_t)v[u].w : (uint32_t)v[u].z);
-                atomicAdd(cell + (CTOT - first_off), swap_ws ? (uint32_t)v[u].z : (uint32_t)v[u].w);
+                // The lane's first word is W or S of its column (lane_off holds which); the other one is CTOT words
+                // away in the same row, i.e. the same byte offset with bit log2(4 CTOT) flipped (the row offset is a
+                // multiple of 8 CTOT and the lane's part is below it), so the second address costs one instruction.
+                uint32_t* cell2 = reinterpret_cast<uint32_t*>(hbytes + (off ^ (uint32_t)(CTOT * 4)));
+                // (byte permutes with a per-lane selector: a conditional here is compiled into divergent branches)
+                atomicAdd(cell, __byte_perm((uint32_t)v[u].z, (uint32_t)v[u].w, sel_first));
+                atomicAdd(cell2, __byte_perm((uint32_t)v[u].z, (uint32_t)v[u].w, sel_second));
               }
             }
           }
