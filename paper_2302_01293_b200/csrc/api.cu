@@ -194,7 +194,8 @@ extern "C" int qlp_bls_create(const qlp_bls_config* cfg, qlp_bls_ctx** out) {
                                  kFitSmemBytes) == cudaSuccess;
   QLP_ATTR(128); QLP_ATTR(64); QLP_ATTR(32); QLP_ATTR(16); QLP_ATTR(8); QLP_ATTR(4); QLP_ATTR(2); QLP_ATTR(1);
   if (!attr_ok ||
-      cudaFuncSetAttribute(snr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
+      cudaFuncSetAttribute(snr_kernel<kSnrThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess ||
+      cudaFuncSetAttribute(snr_kernel<kSnrThreadsLong>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSel * 256 * 4) != cudaSuccess) {
     cudaGetLastError(); delete ctx; return QLP_BLS_ECUDA;
   }
   if (cudaMallocHost((void**)&ctx->totals_host, 8 * sizeof(int64_t)) != cudaSuccess) {
@@ -496,10 +497,21 @@ extern "C" int qlp_bls_snr(qlp_bls_ctx* ctx, int64_t n_stars, const int64_t* row
   QLP_TRY(ctx->star_order.ensure((size_t)n_stars * sizeof(int32_t)));
   star_order_kernel<<<1, 1024, 0, st>>>(n_stars, grid, (int32_t*)ctx->star_order.p);
   QLP_TRY(launch_ok(ctx));
-  snr_kernel<<<(unsigned)n_stars, kSnrThreads, kMaxSel * 256 * 4, st>>>(
+  // two launches side by side: the long grids with 1,024 threads per star on a side stream, the rest with 256
+  QLP_TRY(ensure_side_streams(ctx));
+  CUDA_TRY(cudaEventRecord(ctx->fork_ev, st));
+  CUDA_TRY(cudaStreamWaitEvent(ctx->side[0], ctx->fork_ev, 0));
+  snr_kernel<kSnrThreadsLong><<<(unsigned)n_stars, kSnrThreadsLong, kMaxSel * 256 * 4, ctx->side[0]>>>(
       ctx->prm, n_stars, row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, grid, freq_ptr, sr, best,
       snr, peaks, (const int32_t*)ctx->star_order.p);
-  return launch_ok(ctx);
+  QLP_TRY(launch_ok(ctx));
+  snr_kernel<kSnrThreads><<<(unsigned)n_stars, kSnrThreads, kMaxSel * 256 * 4, st>>>(
+      ctx->prm, n_stars, row_ptr, (const Point*)ctx->pts.p, (const StarPrep*)ctx->prep.p, grid, freq_ptr, sr, best,
+      snr, peaks, (const int32_t*)ctx->star_order.p);
+  QLP_TRY(launch_ok(ctx));
+  CUDA_TRY(cudaEventRecord(ctx->side_done[0], ctx->side[0]));
+  CUDA_TRY(cudaStreamWaitEvent(st, ctx->side_done[0], 0));
+  return QLP_BLS_OK;
 }
 
 // ---- O7: per-peak statistics --------------------------------------------------------------------------

@@ -14,7 +14,9 @@
 
 namespace qlp {
 
-constexpr int kSnrThreads = 256;
+constexpr int kSnrThreads = 256;        // threads per CTA (= per star) of the S4 kernel ...
+constexpr int kSnrThreadsLong = 1024;   // ... and for stars with at least kSnrLongGrid frequencies (a second launch)
+constexpr int64_t kSnrLongGrid = 32768;
 constexpr int kMaxSturges = 31;
 constexpr int kMaxSel = 2 * (kMaxSturges + 1);
 
@@ -35,9 +37,9 @@ struct SnrShared {
   double cx[kMaxSturges + 1], cy[kMaxSturges + 1];
   int32_t nk;
   double med, sigma;
-  double red_v[kSnrThreads / 32];
-  int64_t red_k[kSnrThreads / 32];
-  int32_t red_t[kSnrThreads / 32];
+  double red_v[kSnrThreadsLong / 32];
+  int64_t red_k[kSnrThreadsLong / 32];
+  int32_t red_t[kSnrThreadsLong / 32];
   double win_v; int64_t win_k; int32_t win_t;
   int64_t peak_k[kMaxTopK];
   double peak_v[kMaxTopK];
@@ -48,14 +50,14 @@ struct SnrShared {
 // Runs the radix select for selections [sel0, sel1).  key_of(k) gives the 32-bit key of element k;
 // selection `sel` looks at elements [lo(sel), hi(sel)).  On return sh.prefix[sel] is the key of the
 // wanted order statistic.
-template <typename KeyFn>
+template <int NT, typename KeyFn>
 __device__ void radix_select(SnrShared& sh, uint32_t* hist, int n_sel, int64_t n, int N, bool per_bin, KeyFn key_of) {
   const int tid = threadIdx.x;
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 24 - 8 * pass;
-    for (int i = tid; i < n_sel * 256; i += kSnrThreads) hist[i] = 0u;
+    for (int i = tid; i < n_sel * 256; i += NT) hist[i] = 0u;
     __syncthreads();
-    for (int64_t k = tid; k < n; k += kSnrThreads) {
+    for (int64_t k = tid; k < n; k += NT) {
       const uint32_t key = key_of(k);
       const uint32_t hi = (pass == 0) ? 0u : (key >> (shift + 8));
       const uint32_t dg = (key >> shift) & 255u;

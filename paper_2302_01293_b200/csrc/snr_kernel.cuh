@@ -28,7 +28,12 @@ __global__ void __launch_bounds__(1024) star_order_kernel(int64_t n_stars, const
   for (int64_t s = threadIdx.x; s < n_stars; s += blockDim.x) order[atomicAdd(&base[bucket(s)], 1u)] = (int32_t)s;
 }
 
-__global__ void __launch_bounds__(kSnrThreads) snr_kernel(
+// NT threads per star: the launch with NT = kSnrThreadsLong takes the stars with at least kSnrLongGrid frequencies, the
+// one with NT = kSnrThreads the others (each CTA of the wrong launch leaves at once).  On config 5 the kernel's time
+// is set by its longest grids (one CTA makes ~9 passes over up to 3 MB of SR): 14.5 -> 8.8 ms with 1,024 threads for
+// those; small grids are faster with 256 (config 2: +0.7 % of a step with 1,024 for all).
+template <int NT>
+__global__ void __launch_bounds__(NT) snr_kernel(
     Params prm, int64_t n_stars, const int64_t* __restrict__ row_ptr, const Point* __restrict__ pts,
     const StarPrep* __restrict__ prep, const qlp_bls_star_grid* __restrict__ grid,
     const int64_t* __restrict__ freq_ptr, const float* __restrict__ sr, const uint32_t* __restrict__ best,
@@ -41,8 +46,9 @@ __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
   const int K = prm.top_k;
   const qlp_bls_star_grid g = grid[s];
   const int64_t fo = freq_ptr[s], n = freq_ptr[s + 1] - fo;
+  if ((n >= kSnrLongGrid) != (NT == kSnrThreadsLong)) return;  // the other launch's star
   qlp_bls_peak* pk = peaks + s * K;
-  for (int i = tid; i < K; i += kSnrThreads) {
+  for (int i = tid; i < K; i += NT) {
     qlp_bls_peak p;
     p.k = -1; p.freq = 0.0; p.period = 0.0; p.t0 = 0.0; p.sr = 0.f; p.snr = 0.f; p.q = 0.f; p.depth = 0.f;
     p.m = 0; p.j = 0; p.nb = 0; p.status = 1;
@@ -80,7 +86,7 @@ __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
     sh.prefix[tid] = 0u;
   }
   __syncthreads();
-  radix_select(sh, sel_hist, n_sel, n, N, true, [&](int64_t k) { return f2key(srs[k]); });
+  radix_select<NT>(sh, sel_hist, n_sel, n, N, true, [&](int64_t k) { return f2key(srs[k]); });
   if (tid == 0) {
     int nk = 0;
     for (int b = 0; b < N; ++b) {
@@ -97,7 +103,7 @@ __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
   const double med = sh.med;
   if (tid < 2) { sh.active[tid] = 1; sh.rank[tid] = tid ? n / 2 : (n - 1) / 2; sh.prefix[tid] = 0u; }
   __syncthreads();
-  radix_select(sh, sel_hist, 2, n, N, false, [&](int64_t k) { return f2key((float)fabs(dsub((double)srs[k], med))); });
+  radix_select<NT>(sh, sel_hist, 2, n, N, false, [&](int64_t k) { return f2key((float)fabs(dsub((double)srs[k], med))); });
   if (tid == 0) sh.sigma = dmul(1.4826, dmul(0.5, dadd((double)key2f(sh.prefix[0]), (double)key2f(sh.prefix[1]))));
   __syncthreads();
   const double sigma = sh.sigma;
@@ -109,7 +115,7 @@ __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
 #pragma unroll
   for (int i = 0; i < kMaxTopK; ++i) { tv[i] = -1.0e300; tk[i] = -1; }
   // contiguous chunk per thread so that neighbours are mostly the thread's own values
-  const int64_t per = (n + kSnrThreads - 1) / kSnrThreads;
+  const int64_t per = (n + NT - 1) / NT;
   const int64_t ka = (int64_t)tid * per, kb_ = (ka + per < n) ? ka + per : n;
   if (ka < kb_) {
     double prev = (ka > 0) ? snr_at(ka - 1) : 0.0;
@@ -145,7 +151,7 @@ __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
     __syncthreads();
     if (tid == 0) {
       double bv = sh.red_v[0]; int64_t bk = sh.red_k[0]; int bt = sh.red_t[0];
-      for (int w = 1; w < kSnrThreads / 32; ++w) {
+      for (int w = 1; w < NT / 32; ++w) {
         double v2 = sh.red_v[w]; int64_t k2 = sh.red_k[w];
         if (k2 >= 0 && (bk < 0 || v2 > bv || (v2 == bv && k2 < bk))) { bv = v2; bk = k2; bt = sh.red_t[w]; }
       }
@@ -176,7 +182,7 @@ __global__ void __launch_bounds__(kSnrThreads) snr_kernel(
     if (tid == 0) { sh.accW = 0ull; sh.accS = 0ll; }
     __syncthreads();
     unsigned long long aw = 0ull; long long as = 0ll;
-    for (int64_t p = tid; p < np; p += kSnrThreads) {
+    for (int64_t p = tid; p < np; p += NT) {
       const Point pt = pts[pa + p];
       int b = bin_of(f, pt.tau, dnb, Kc) - j;
       if (b < 0) b += nb;
