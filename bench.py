@@ -52,7 +52,7 @@ N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum over the foldscan launches of ONE step of a named workload, from an
 # `ncu --set full` capture kept under profiles/ (not measured in this run: a run under ncu is never a bench value).
 NCU_TRAFFIC = {
-    (5, 4000): (7.829e9, "profiles/r2_launches.md (ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum over the "
+    (5, 4000): (7.837e9, "profiles/r2_launches.md (ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum over the "
                          "nine foldscan launches of one step of this workload)"),
     (2, 1000): (719.3e6, "profiles/r1_foldscan_ncu.txt (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum "
                          "over the foldscan launches of one step)"),
